@@ -1,0 +1,792 @@
+// sop.cu -- host side of the C ABI in include/sop.h: validation, static tables, workspace carving, launch
+// schedule (list invariant), getters.  All arithmetic of the hot path is in the kernels (sop_kernels.cuh).
+#include "../../include/sop.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <string>
+#include <vector>
+
+#include "sop_kernels.cuh"
+#include "sop_persistent.cuh"
+
+using namespace sop;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+struct Plan {                     // everything that depends only on (topology, native coords, params, n_traj)
+  int N = 0, T = 0;
+  std::vector<int> perm, iperm;   // perm[internal] = caller index; iperm[caller] = internal
+  int cap_b = 1, cap_nb = 0, cap_pl = 0;
+  bool static_l1 = false, comp = false, reorder = false;
+  int lanes = 1, block = 256, mode = 1;
+  int max_cells = 1;
+  size_t n_nat_entries = 0, n_excl = 0;
+  int energy_blocks = 1;
+  // workspace offsets
+  size_t off_pos0, off_pos1, off_carry, off_force, off_bond, off_natptr, off_nattab, off_nateps, off_exclptr,
+      off_exclidx, off_adotn, off_plcnt, off_plidx, off_nbcnt, off_nbidx, off_bbox, off_grid, off_cellof,
+      off_cellcnt, off_cellstart, off_cellbead, off_flags, off_epart, off_eout, off_bar, total;
+};
+
+size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+int fail(int code, const std::string &msg, sop_handle *h = nullptr);
+
+#define CUDA_OK(call)                                                                                   \
+  do {                                                                                                  \
+    cudaError_t e_ = (call);                                                                            \
+    if (e_ != cudaSuccess)                                                                              \
+      return fail(SOP_E_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_), h);                   \
+  } while (0)
+
+}  // namespace
+
+struct sop_handle {
+  Plan plan;
+  SysDev S;
+  sop_params prm;
+  cudaStream_t stream = nullptr;
+  int cur = 0;                    // index of the current time layer
+  int64_t step = 0, l1_built_at = 0, l2_built_at = 0;
+  uint64_t launches = 0;
+  char *ws = nullptr;
+  std::string last_error;
+  int coop_blocks = 0;            // persistent kernel: grid size (co-resident)
+  int coop_block_size = 0;
+  int num_sms = 0;
+  unsigned *S_bar = nullptr;      // grid-barrier counter of the persistent kernel
+  std::vector<uint32_t> tag;      // [N] host copy of the coordinate tags (internal order)
+  float4 *stage = nullptr;        // pinned host staging buffer [T][N] for coordinate transfers
+  // optional kernel timing (sop_set_profiling): event pairs around groups of launches of one kind
+  struct Span { cudaEvent_t a, b; int kind; int64_t steps; };
+  bool profiling = false;
+  std::vector<Span> spans;
+  int open_kind = -1;
+  double prof_ms[3] = {0, 0, 0};
+  int64_t prof_n[3] = {0, 0, 0}, prof_steps = 0;
+};
+
+namespace {
+
+int fail(int code, const std::string &msg, sop_handle *h) {
+  g_last_error = msg;
+  if (h) h->last_error = msg;
+  return code;
+}
+
+// ---- host-side neighbour statistics of the native structure (sizing only; not on the hot path) ----------
+int max_neighbors(const std::vector<double> &x, int N, double R) {
+  if (!std::isfinite(R)) return N - 1;
+  double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+  for (int i = 0; i < N; ++i)
+    for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], x[3 * i + a]); hi[a] = std::max(hi[a], x[3 * i + a]); }
+  int n[3];
+  for (int a = 0; a < 3; ++a) n[a] = std::max(1, std::min(1024, (int)std::floor((hi[a] - lo[a]) / R) + 1));
+  double edge[3];
+  for (int a = 0; a < 3; ++a) edge[a] = std::max(R, (hi[a] - lo[a]) / n[a] * (1 + 1e-9) + 1e-9);
+  auto cell = [&](int i, int a) { return std::min(n[a] - 1, std::max(0, (int)std::floor((x[3 * i + a] - lo[a]) / edge[a]))); };
+  size_t ncell = (size_t)n[0] * n[1] * n[2];
+  std::vector<int> start(ncell + 1, 0), of(N), order(N);
+  for (int i = 0; i < N; ++i) { of[i] = (cell(i, 2) * n[1] + cell(i, 1)) * n[0] + cell(i, 0); start[of[i] + 1]++; }
+  for (size_t c = 0; c < ncell; ++c) start[c + 1] += start[c];
+  std::vector<int> fill(start.begin(), start.end() - 1);
+  for (int i = 0; i < N; ++i) order[fill[of[i]]++] = i;
+  const double R2 = R * R;
+  int best = 0;
+  for (int i = 0; i < N; ++i) {
+    int cx = cell(i, 0), cy = cell(i, 1), cz = cell(i, 2), cnt = 0;
+    for (int z = std::max(0, cz - 1); z <= std::min(n[2] - 1, cz + 1); ++z)
+      for (int y = std::max(0, cy - 1); y <= std::min(n[1] - 1, cy + 1); ++y)
+        for (int xx = std::max(0, cx - 1); xx <= std::min(n[0] - 1, cx + 1); ++xx) {
+          int c = (z * n[1] + y) * n[0] + xx;
+          for (int q = start[c]; q < start[c + 1]; ++q) {
+            int j = order[q];
+            double dx = x[3 * i] - x[3 * j], dy = x[3 * i + 1] - x[3 * j + 1], dz = x[3 * i + 2] - x[3 * j + 2];
+            cnt += (dx * dx + dy * dy + dz * dz < R2);
+          }
+        }
+    best = std::max(best, cnt - 1);
+  }
+  return best;
+}
+
+uint32_t part1by2(uint32_t v) {   // spread the low 10 bits of v
+  v &= 0x3FF;
+  v = (v | (v << 16)) & 0x030000FF;
+  v = (v | (v << 8)) & 0x0300F00F;
+  v = (v | (v << 4)) & 0x030C30C3;
+  v = (v | (v << 2)) & 0x09249249;
+  return v;
+}
+
+int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int32_t T, Plan &pl) {
+  if (!tp || !xyz || !p || T < 1) return fail(SOP_E_ARG, "null argument or n_traj < 1");
+  const int N = tp->n_beads;
+  if (N < 1 || N > (int)TAG_ID_MASK) return fail(SOP_E_ARG, "n_beads out of range");
+  if ((long long)N * T > 0x7FFFFFF0LL) return fail(SOP_E_ARG, "n_beads * n_traj too large");
+  if (p->nb_interval < 1 || p->pl_interval < 1 || p->pl_interval % p->nb_interval != 0)
+    return fail(SOP_E_ARG, "pl_interval must be a positive multiple of nb_interval");
+  if (!(p->R_nb > 0) || !(p->R_pl >= p->R_nb) || !(p->R0 > 0) || !(p->dt_over_zeta >= 0) || !(p->kT >= 0))
+    return fail(SOP_E_ARG, "bad cutoffs / R0 / dt_over_zeta / kT");
+  for (int q = 0; q < 3 * N; ++q)
+    if (!std::isfinite(xyz[q])) return fail(SOP_E_ARG, "non-finite native coordinate");
+  pl.N = N; pl.T = T;
+  pl.static_l1 = std::isinf(p->R_pl);
+
+  std::vector<double> x(3 * (size_t)N);
+  double maxabs = 0;
+  for (size_t q = 0; q < 3 * (size_t)N; ++q) { x[q] = xyz[q]; maxabs = std::max(maxabs, std::fabs(x[q])); }
+  pl.comp = p->compensated == 1 || (p->compensated == 0 && maxabs > 512.0);
+
+  // internal bead order: Morton order of 8 A cells of the native structure (gather locality), ties by index
+  pl.reorder = p->reorder == 1;
+  pl.perm.resize(N); pl.iperm.resize(N);
+  for (int i = 0; i < N; ++i) pl.perm[i] = i;
+  if (pl.reorder) {
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int i = 0; i < N; ++i)
+      for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], x[3 * i + a]); hi[a] = std::max(hi[a], x[3 * i + a]); }
+    double ext = std::max({hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2], 1.0});
+    double cellw = std::max(8.0, ext / 1023.0);
+    std::vector<uint32_t> key(N);
+    for (int i = 0; i < N; ++i) {
+      uint32_t c[3];
+      for (int a = 0; a < 3; ++a) c[a] = (uint32_t)std::min(1023.0, std::floor((x[3 * i + a] - lo[a]) / cellw));
+      key[i] = part1by2(c[0]) | (part1by2(c[1]) << 1) | (part1by2(c[2]) << 2);
+    }
+    std::stable_sort(pl.perm.begin(), pl.perm.end(), [&](int a, int b) { return key[a] < key[b]; });
+  }
+  for (int i = 0; i < N; ++i) pl.iperm[pl.perm[i]] = i;
+
+  // row capacities (the paper's M)
+  std::vector<int> deg(N, 0);
+  for (int b = 0; b < tp->n_bonds; ++b) {
+    int i = tp->bonds[2 * b], j = tp->bonds[2 * b + 1];
+    if (i < 0 || j >= N || i >= j) return fail(SOP_E_ARG, "bond out of range or not i<j");
+    deg[i]++; deg[j]++;
+  }
+  pl.cap_b = std::max(1, *std::max_element(deg.begin(), deg.end()));
+  for (int c = 0; c < tp->n_native; ++c) {
+    int i = tp->native[2 * c], j = tp->native[2 * c + 1];
+    if (i < 0 || j >= N || i >= j) return fail(SOP_E_ARG, "native pair out of range or not i<j");
+  }
+  pl.n_nat_entries = 2 * (size_t)tp->n_native;
+  pl.n_excl = 2 * ((size_t)tp->n_native + (size_t)tp->n_bonds);
+  auto cap_of = [&](int requested, double R) {
+    if (requested > 0) return (requested + 3) / 4 * 4;
+    int m = max_neighbors(x, N, R);
+    if (!std::isfinite(R)) return (std::max(m, 1) + 3) / 4 * 4;
+    return ((int)(m * 1.15) + 8 + 3) / 4 * 4;
+  };
+  pl.cap_nb = cap_of(p->cap_nb, p->R_nb);
+  pl.cap_pl = cap_of(p->cap_pl, p->R_pl);
+  if (pl.static_l1 && (size_t)N * pl.cap_pl > (size_t)1 << 30)
+    return fail(SOP_E_ARG, "R_pl = +inf needs an N x N pair list: N too large, give a finite R_pl");
+
+  // cell grid capacity: the native bounding box, with room for the structure to grow 4x per axis sum
+  if (!pl.static_l1) {
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int i = 0; i < N; ++i)
+      for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], x[3 * i + a]); hi[a] = std::max(hi[a], x[3 * i + a]); }
+    double edge = (double)p->R_pl * 1.001, tot = 1;
+    for (int a = 0; a < 3; ++a) tot *= std::floor((hi[a] - lo[a]) / edge) + 1;
+    pl.max_cells = (int)std::min(4.0e6, std::max(64.0, tot * 4.0));
+  }
+
+  // launch shape
+  const long long inst = (long long)N * T;
+  int lanes = p->lanes_per_bead;
+  if (lanes == 0) {
+    lanes = 32;
+    while (lanes > 1 && inst * lanes > 1200000LL) lanes >>= 1;   // ~4 resident threads' worth of the chip
+  }
+  if (lanes != 1 && lanes != 2 && lanes != 4 && lanes != 8 && lanes != 16 && lanes != 32)
+    return fail(SOP_E_ARG, "lanes_per_bead must be 0 or a power of two <= 32");
+  pl.lanes = lanes;
+  pl.block = p->block_size > 0 ? p->block_size : 256;
+  if (pl.block % 32 || pl.block > 1024) return fail(SOP_E_ARG, "block_size must be a multiple of 32, <= 1024");
+  pl.mode = p->mode == 0 ? 1 : p->mode;
+  if (pl.mode != 1 && pl.mode != 2) return fail(SOP_E_ARG, "mode must be 0, 1 or 2");
+  pl.energy_blocks = (int)std::min<long long>(64, ((long long)N * 8 + 255) / 256);
+
+  // workspace
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+  const size_t I = (size_t)inst;
+  pl.off_pos0 = take(I * 16); pl.off_pos1 = take(I * 16);
+  pl.off_carry = take(pl.comp ? I * 16 : 0);
+  pl.off_force = take(I * 16);
+  pl.off_bond = take((size_t)N * pl.cap_b * 8);
+  pl.off_natptr = take(((size_t)N + 1) * 4);
+  pl.off_nattab = take(pl.n_nat_entries * 8);
+  pl.off_nateps = take(tp->native_eps ? pl.n_nat_entries * 4 : 0);
+  pl.off_exclptr = take(((size_t)N + 1) * 4);
+  pl.off_exclidx = take(pl.n_excl * 4);
+  pl.off_adotn = take(p->n_pulled > 0 ? (size_t)N * 4 : 0);
+  const size_t rows1 = pl.static_l1 ? (size_t)N : I;
+  pl.off_plcnt = take(rows1 * 4); pl.off_plidx = take(rows1 * pl.cap_pl * 4);
+  pl.off_nbcnt = take(I * 4); pl.off_nbidx = take(I * pl.cap_nb * 4);
+  pl.off_bbox = take((size_t)T * 6 * 4); pl.off_grid = take((size_t)T * sizeof(GridDev));
+  pl.off_cellof = take(pl.static_l1 ? 0 : I * 4);
+  pl.off_cellcnt = take(pl.static_l1 ? 0 : (size_t)T * pl.max_cells * 4);
+  pl.off_cellstart = take(pl.static_l1 ? 0 : (size_t)T * ((size_t)pl.max_cells + 1) * 4);
+  pl.off_cellbead = take(pl.static_l1 ? 0 : I * 4);
+  pl.off_flags = take(64);
+  pl.off_epart = take((size_t)T * pl.energy_blocks * 5 * 8);
+  pl.off_eout = take((size_t)T * 6 * 8);
+  pl.off_bar = take(256);
+  pl.total = o;
+  return SOP_OK;
+}
+
+enum { SPAN_STEP = 0, SPAN_FILTER = 1, SPAN_L1 = 2 };
+
+void span_close(sop_handle *h) {
+  if (h->open_kind < 0) return;
+  cudaEventRecord(h->spans.back().b, h->stream);
+  h->open_kind = -1;
+}
+// open (or extend) a timed span of `kind`; consecutive launches of the same kind share one event pair
+void span_begin(sop_handle *h, int kind, int64_t steps) {
+  if (!h->profiling) return;
+  if (h->open_kind == kind) { h->spans.back().steps += steps; return; }
+  span_close(h);
+  sop_handle::Span sp;
+  cudaEventCreate(&sp.a); cudaEventCreate(&sp.b);
+  sp.kind = kind; sp.steps = steps;
+  cudaEventRecord(sp.a, h->stream);
+  h->spans.push_back(sp);
+  h->open_kind = kind;
+}
+
+template <int G>
+void launch_step_g(sop_handle *h, bool forces) {
+  const SysDev &S = h->S;
+  const long long threads = (long long)S.n_inst * G;
+  const int block = h->plan.block;
+  const unsigned grid = (unsigned)((threads + block - 1) / block);
+  const unsigned long long step = (unsigned long long)h->step;
+  if (forces) k_step<G, false, true><<<grid, block, 0, h->stream>>>(S, h->cur, step);
+  else if (h->plan.comp) k_step<G, true, false><<<grid, block, 0, h->stream>>>(S, h->cur, step);
+  else k_step<G, false, false><<<grid, block, 0, h->stream>>>(S, h->cur, step);
+  h->launches++;
+}
+
+void launch_step(sop_handle *h, bool forces) {
+  switch (h->plan.lanes) {
+    case 1: launch_step_g<1>(h, forces); break;
+    case 2: launch_step_g<2>(h, forces); break;
+    case 4: launch_step_g<4>(h, forces); break;
+    case 8: launch_step_g<8>(h, forces); break;
+    case 16: launch_step_g<16>(h, forces); break;
+    default: launch_step_g<32>(h, forces); break;
+  }
+}
+
+void launch_filter(sop_handle *h) {
+  const SysDev &S = h->S;
+  span_begin(h, SPAN_FILTER, 1);
+  const long long threads = (long long)S.n_inst * 32;
+  k_filter<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(S, h->cur);
+  h->launches++;
+  h->l2_built_at = h->step;
+}
+
+int launch_build_l1(sop_handle *h) {
+  const SysDev &S = h->S;
+  cudaStream_t st = h->stream;
+  span_begin(h, SPAN_L1, 1);
+  if (S.static_l1) {
+    k_build_l1_static<<<(unsigned)(((long long)S.N * 32 + 255) / 256), 256, 0, st>>>(S);
+    h->launches++;
+  } else {
+    k_bbox_init<<<(S.T * 6 + 255) / 256, 256, 0, st>>>(S);
+    dim3 gb((unsigned)std::min(64, (S.N + 255) / 256), (unsigned)S.T);
+    k_bbox<<<gb, 256, 0, st>>>(S, h->cur);
+    k_grid_setup<<<(S.T + 127) / 128, 128, 0, st>>>(S);
+    CUDA_OK(cudaMemsetAsync(S.cell_cnt, 0, (size_t)S.T * S.max_cells * 4, st));
+    const unsigned gi = (unsigned)((S.n_inst + 255) / 256);
+    k_cell_count<<<gi, 256, 0, st>>>(S, h->cur);
+    k_cell_scan<<<S.T, 1024, 0, st>>>(S);
+    k_cell_fill<<<gi, 256, 0, st>>>(S);
+    dim3 gs((unsigned)std::min(1024, (S.max_cells * 32 + 255) / 256), (unsigned)S.T);
+    k_cell_sort<<<gs, 256, 0, st>>>(S);
+    k_build_l1<<<(unsigned)(((long long)S.n_inst * 32 + 255) / 256), 256, 0, st>>>(S, h->cur);
+    h->launches += 8;
+  }
+  h->l1_built_at = h->step;
+  return SOP_OK;
+}
+
+int check_launch(sop_handle *h, const char *what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(SOP_E_CUDA, std::string(what) + ": " + cudaGetErrorString(e), h);
+  return SOP_OK;
+}
+
+int read_flags(sop_handle *h) {
+  int flags = 0;
+  CUDA_OK(cudaMemcpyAsync(&flags, h->S.flags, 4, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_OK(cudaStreamSynchronize(h->stream));
+  if (!flags) return SOP_OK;
+  CUDA_OK(cudaMemsetAsync(h->S.flags, 0, 4, h->stream));
+  if (flags & FLAG_NONFINITE) return fail(SOP_E_NONFINITE, "non-finite coordinate or bead inside the indenter", h);
+  if (flags & FLAG_FENE) return fail(SOP_E_FENE, "a bond reached |r - r0| >= R0", h);
+  if (flags & FLAG_PL_OVERFLOW) return fail(SOP_E_LIST_OVERFLOW, "pair-list row exceeded cap_pl", h);
+  return fail(SOP_E_LIST_OVERFLOW, "neighbor-list row exceeded cap_nb", h);
+}
+
+
+template <int G, bool COMP>
+const void *persist_fn() { return (const void *)k_persist<G, COMP>; }
+
+const void *persist_kernel(int lanes, bool comp) {
+  switch (lanes) {
+    case 1: return comp ? persist_fn<1, true>() : persist_fn<1, false>();
+    case 2: return comp ? persist_fn<2, true>() : persist_fn<2, false>();
+    case 4: return comp ? persist_fn<4, true>() : persist_fn<4, false>();
+    case 8: return comp ? persist_fn<8, true>() : persist_fn<8, false>();
+    case 16: return comp ? persist_fn<16, true>() : persist_fn<16, false>();
+    default: return comp ? persist_fn<32, true>() : persist_fn<32, false>();
+  }
+}
+
+// grid of the persistent kernel: every block co-resident (cooperative launch), no more blocks than there is work
+int persistent_prepare(sop_handle *h) {
+  const Plan &pl = h->plan;
+  int block = h->prm.block_size > 0 ? h->prm.block_size : 512;
+  int occ = 0;
+  CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, persist_kernel(pl.lanes, pl.comp), block, 0));
+  if (occ < 1) return fail(SOP_E_CUDA, "persistent kernel does not fit on an SM", h);
+  int coop = 0, dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+  if (!coop) return fail(SOP_E_CUDA, "device cannot do cooperative launches", h);
+  const long long want = ((long long)h->S.n_inst * pl.lanes + block - 1) / block;
+  h->coop_blocks = (int)std::max<long long>(1, std::min<long long>((long long)h->num_sms * std::min(occ, 2), want));
+  h->coop_block_size = block;
+  return SOP_OK;
+}
+
+int persistent_launch(sop_handle *h, int n, bool filter_last) {
+  CUDA_OK(cudaMemsetAsync(h->S_bar, 0, 4, h->stream));
+  span_close(h);
+  span_begin(h, SPAN_STEP, n);
+  SysDev S = h->S;
+  int cur = h->cur;
+  unsigned long long step0 = (unsigned long long)h->step;
+  int nb = h->prm.nb_interval, fl = filter_last ? 1 : 0;
+  unsigned *bar = h->S_bar;
+  void *args[] = {&S, &cur, &step0, &n, &nb, &fl, &bar};
+  CUDA_OK(cudaLaunchCooperativeKernel(persist_kernel(h->plan.lanes, h->plan.comp), dim3(h->coop_blocks),
+                                      dim3(h->coop_block_size), args, 0, h->stream));
+  h->launches++;
+  return SOP_OK;
+}
+
+int rebuild_lists(sop_handle *h) {
+  int rc = launch_build_l1(h);
+  if (rc) return rc;
+  launch_filter(h);
+  span_close(h);
+  return check_launch(h, "list rebuild");
+}
+
+}  // namespace
+
+// =====================================================================================================
+extern "C" {
+
+const char *sop_last_error(sop_handle *h) { return h ? h->last_error.c_str() : g_last_error.c_str(); }
+
+int sop_query_workspace(const sop_topology *topo, const float *native_xyz, const sop_params *params, int32_t n_traj,
+                        size_t *bytes_out) {
+  if (!bytes_out) return fail(SOP_E_ARG, "bytes_out is null");
+  Plan pl;
+  int rc = make_plan(topo, native_xyz, params, n_traj, pl);
+  if (rc) return rc;
+  *bytes_out = pl.total;
+  return SOP_OK;
+}
+
+int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params *p, int32_t n_traj,
+               void *d_workspace, size_t workspace_bytes, sop_handle **out) {
+  if (!out) return fail(SOP_E_ARG, "out is null");
+  *out = nullptr;
+  sop_handle *h = new sop_handle();
+  Plan &pl = h->plan;
+  int rc = make_plan(tp, native_xyz, p, n_traj, pl);
+  if (rc) { delete h; return rc; }
+  if (!d_workspace || workspace_bytes < pl.total || ((uintptr_t)d_workspace & 255)) {
+    delete h;
+    return fail(SOP_E_ARG, "workspace missing, misaligned or smaller than sop_query_workspace says");
+  }
+  const int N = pl.N, T = pl.T;
+  h->prm = *p;
+  h->prm.fixed = nullptr; h->prm.pulled = nullptr;
+  h->stream = (cudaStream_t)p->stream;
+  h->ws = (char *)d_workspace;
+
+  // ---- static tables in internal order; r0 from the native structure in fp64, rounded to fp32
+  auto X = [&](int caller, int a) { return (double)native_xyz[3 * (size_t)caller + a]; };
+  auto dist = [&](int i, int j) {
+    double dx = X(i, 0) - X(j, 0), dy = X(i, 1) - X(j, 1), dz = X(i, 2) - X(j, 2);
+    return std::sqrt(dx * dx + dy * dy + dz * dz);
+  };
+  std::vector<int2> bond_tab((size_t)N * pl.cap_b, make_int2(-1, 0));
+  std::vector<int> bfill(N, 0);
+  std::vector<std::vector<int>> excl(N);
+  for (int b = 0; b < tp->n_bonds; ++b) {
+    int i = tp->bonds[2 * b], j = tp->bonds[2 * b + 1];
+    float r0 = (float)dist(i, j);
+    int ii = pl.iperm[i], jj = pl.iperm[j];
+    int r0b; memcpy(&r0b, &r0, 4);
+    bond_tab[(size_t)ii * pl.cap_b + bfill[ii]++] = make_int2(jj, r0b);
+    bond_tab[(size_t)jj * pl.cap_b + bfill[jj]++] = make_int2(ii, r0b);
+    excl[ii].push_back(jj); excl[jj].push_back(ii);
+  }
+  struct NatE { int j; float r0sq; float eps; };
+  std::vector<std::vector<NatE>> nat(N);
+  for (int c = 0; c < tp->n_native; ++c) {
+    int i = tp->native[2 * c], j = tp->native[2 * c + 1];
+    float r0 = (float)dist(i, j);
+    float r0sq = (float)((double)r0 * (double)r0);
+    float eps = tp->native_eps ? tp->native_eps[c] : p->eps_native;
+    int ii = pl.iperm[i], jj = pl.iperm[j];
+    nat[ii].push_back({jj, r0sq, eps}); nat[jj].push_back({ii, r0sq, eps});
+    excl[ii].push_back(jj); excl[jj].push_back(ii);
+  }
+  std::vector<int> nat_ptr(N + 1, 0), excl_ptr(N + 1, 0);
+  std::vector<int2> nat_tab; nat_tab.reserve(pl.n_nat_entries);
+  std::vector<float> nat_eps; std::vector<int> excl_idx; excl_idx.reserve(pl.n_excl);
+  for (int i = 0; i < N; ++i) {
+    std::sort(nat[i].begin(), nat[i].end(), [](const NatE &a, const NatE &b) { return a.j < b.j; });
+    for (auto &e : nat[i]) { int b; memcpy(&b, &e.r0sq, 4); nat_tab.push_back(make_int2(e.j, b)); nat_eps.push_back(e.eps); }
+    nat_ptr[i + 1] = (int)nat_tab.size();
+    std::sort(excl[i].begin(), excl[i].end());
+    for (size_t q = 0; q < excl[i].size(); ++q) {
+      if (excl[i][q] == i || (q && excl[i][q] == excl[i][q - 1])) {
+        delete h;
+        return fail(SOP_E_ARG, "duplicate pair, self pair, or a bond that is also a native contact");
+      }
+      excl_idx.push_back(excl[i][q]);
+    }
+    excl_ptr[i + 1] = (int)excl_idx.size();
+  }
+
+  // ---- tags, anchors, initial coordinates
+  std::vector<uint32_t> &tag = h->tag;
+  tag.resize(N);
+  for (int i = 0; i < N; ++i) tag[i] = (uint32_t)pl.perm[i];
+  for (int q = 0; q < p->n_fixed; ++q) {
+    if (!p->fixed || p->fixed[q] < 0 || p->fixed[q] >= N) { delete h; return fail(SOP_E_ARG, "fixed bead out of range"); }
+    tag[pl.iperm[p->fixed[q]]] |= TAG_FIXED;
+  }
+  double nrm[3] = {p->pull_dir[0], p->pull_dir[1], p->pull_dir[2]};
+  std::vector<float> adotn(N, 0.f);
+  for (int q = 0; q < p->n_pulled; ++q) {
+    if (!p->pulled || p->pulled[q] < 0 || p->pulled[q] >= N) { delete h; return fail(SOP_E_ARG, "pulled bead out of range"); }
+    int c = p->pulled[q], ii = pl.iperm[c];
+    tag[ii] |= TAG_PULLED;
+    adotn[ii] = (float)(X(c, 0) * nrm[0] + X(c, 1) * nrm[1] + X(c, 2) * nrm[2]);
+  }
+  std::vector<float4> pos0((size_t)N * T);
+  for (int t = 0; t < T; ++t)
+    for (int ii = 0; ii < N; ++ii) {
+      int c = pl.perm[ii];
+      float w; memcpy(&w, &tag[ii], 4);
+      pos0[(size_t)t * N + ii] = make_float4(native_xyz[3 * (size_t)c], native_xyz[3 * (size_t)c + 1], native_xyz[3 * (size_t)c + 2], w);
+    }
+
+  // ---- device view
+  SysDev &S = h->S;
+  memset(&S, 0, sizeof(S));
+  char *w = h->ws;
+  S.N = N; S.T = T; S.n_inst = N * T;
+  S.pos[0] = (float4 *)(w + pl.off_pos0); S.pos[1] = (float4 *)(w + pl.off_pos1);
+  S.carry = pl.comp ? (float4 *)(w + pl.off_carry) : nullptr;
+  S.force = (float4 *)(w + pl.off_force);
+  S.cap_b = pl.cap_b; S.bond_tab = (const int2 *)(w + pl.off_bond);
+  S.nat_ptr = (const int *)(w + pl.off_natptr); S.nat_tab = (const int2 *)(w + pl.off_nattab);
+  S.nat_eps = tp->native_eps ? (const float *)(w + pl.off_nateps) : nullptr;
+  S.excl_ptr = (const int *)(w + pl.off_exclptr); S.excl_idx = (const int *)(w + pl.off_exclidx);
+  S.pull_adotn = p->n_pulled > 0 ? (const float *)(w + pl.off_adotn) : nullptr;
+  S.static_l1 = pl.static_l1; S.cap_pl = pl.cap_pl; S.cap_nb = pl.cap_nb;
+  S.pl_cnt = (int *)(w + pl.off_plcnt); S.pl_idx = (int *)(w + pl.off_plidx);
+  S.nb_cnt = (int *)(w + pl.off_nbcnt); S.nb_idx = (int *)(w + pl.off_nbidx);
+  S.max_cells = pl.max_cells;
+  S.bbox = (float *)(w + pl.off_bbox); S.grid = (GridDev *)(w + pl.off_grid);
+  S.cell_of = (int *)(w + pl.off_cellof); S.cell_cnt = (int *)(w + pl.off_cellcnt);
+  S.cell_start = (int *)(w + pl.off_cellstart); S.cell_bead = (int *)(w + pl.off_cellbead);
+  S.cell_edge = pl.static_l1 ? 1.0f : (float)((double)p->R_pl * 1.001);
+  S.k_fene = p->k_fene; S.R0 = p->R0; S.inv_R0sq = (float)(1.0 / ((double)p->R0 * (double)p->R0));
+  S.eps_native = p->eps_native;
+  const double sig6 = std::pow((double)p->sigma, 6.0);
+  S.c_rep_e = (float)((double)p->eps_rep * sig6); S.c_rep_f = (float)(6.0 * (double)p->eps_rep * sig6);
+  S.R_nb2 = (float)((double)p->R_nb * (double)p->R_nb);
+  S.R_pl2 = pl.static_l1 ? std::numeric_limits<float>::infinity() : (float)((double)p->R_pl * (double)p->R_pl);
+  S.D = p->dt_over_zeta; S.amp = (float)std::sqrt(2.0 * (double)p->kT * (double)p->dt_over_zeta);
+  S.seed_lo = (uint32_t)(p->seed & 0xFFFFFFFFu); S.seed_hi = (uint32_t)(p->seed >> 32);
+  S.traj_offset = p->traj_offset;
+  S.has_pull = p->n_pulled > 0; S.pull_k = p->pull_k; S.pull_v = p->pull_v;
+  S.pull_nx = p->pull_dir[0]; S.pull_ny = p->pull_dir[1]; S.pull_nz = p->pull_dir[2];
+  S.tip_on = p->tip_on != 0; S.tip_R = p->tip_R; S.tip_eps = p->tip_eps;
+  S.tip_sigma6 = (float)std::pow((double)p->tip_sigma, 6.0); S.tip_v = p->tip_v;
+  S.tip_cx = p->tip_c0[0]; S.tip_cy = p->tip_c0[1]; S.tip_cz = p->tip_c0[2];
+  S.tip_nx = p->tip_dir[0]; S.tip_ny = p->tip_dir[1]; S.tip_nz = p->tip_dir[2];
+  S.flags = (int *)(w + pl.off_flags);
+
+  // ---- upload (synchronous copies from pageable host vectors; create is not on the hot path)
+  cudaStream_t st = h->stream;
+  auto up = [&](size_t off, const void *src, size_t bytes) -> cudaError_t {
+    if (!bytes) return cudaSuccess;
+    return cudaMemcpyAsync(w + off, src, bytes, cudaMemcpyHostToDevice, st);
+  };
+  cudaError_t e = cudaSuccess;
+  auto acc = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  acc(cudaMemsetAsync(w + pl.off_flags, 0, 64, st));
+  acc(cudaMemsetAsync(w + pl.off_bar, 0, 256, st));
+  acc(up(pl.off_pos0, pos0.data(), pos0.size() * 16));
+  acc(up(pl.off_pos1, pos0.data(), pos0.size() * 16));
+  if (pl.comp) acc(cudaMemsetAsync(w + pl.off_carry, 0, pos0.size() * 16, st));
+  acc(up(pl.off_bond, bond_tab.data(), bond_tab.size() * 8));
+  acc(up(pl.off_natptr, nat_ptr.data(), nat_ptr.size() * 4));
+  acc(up(pl.off_nattab, nat_tab.data(), nat_tab.size() * 8));
+  if (tp->native_eps) acc(up(pl.off_nateps, nat_eps.data(), nat_eps.size() * 4));
+  acc(up(pl.off_exclptr, excl_ptr.data(), excl_ptr.size() * 4));
+  acc(up(pl.off_exclidx, excl_idx.data(), excl_idx.size() * 4));
+  if (p->n_pulled > 0) acc(up(pl.off_adotn, adotn.data(), adotn.size() * 4));
+  acc(cudaStreamSynchronize(st));
+  if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); delete h; return fail(SOP_E_CUDA, "upload: " + m); }
+
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  h->S_bar = (unsigned *)(w + pl.off_bar);
+  if (pl.mode == 2) {
+    rc = persistent_prepare(h);
+    if (rc) { std::string m = g_last_error; delete h; return fail(rc, m); }
+  }
+
+  h->cur = 0; h->step = 0;
+  rc = rebuild_lists(h);
+  if (!rc) rc = read_flags(h);
+  if (rc) { std::string m = h->last_error; delete h; return fail(rc, m); }
+  *out = h;
+  return SOP_OK;
+}
+
+void sop_destroy(sop_handle *h) {
+  if (!h) return;
+  cudaStreamSynchronize(h->stream);
+  for (auto &sp : h->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+  if (h->stage) cudaFreeHost(h->stage);
+  delete h;
+}
+
+// Kernel timing for the bench: CUDA events on the handle's stream around groups of launches.
+// out[0..2] = ms in {step kernels, L2 filter kernels, L1 build kernels}, out[3..5] = number of such spans,
+// out[6] = Langevin steps covered by the step spans, out[7] = reserved.  Reading synchronises and resets.
+int sop_set_profiling(sop_handle *h, int32_t on) {
+  if (!h) return fail(SOP_E_ARG, "null handle");
+  h->profiling = on != 0;
+  return SOP_OK;
+}
+
+int sop_get_profile(sop_handle *h, double out[8]) {
+  if (!h || !out) return fail(SOP_E_ARG, "null argument", h);
+  span_close(h);
+  CUDA_OK(cudaStreamSynchronize(h->stream));
+  for (auto &sp : h->spans) {
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, sp.a, sp.b);
+    h->prof_ms[sp.kind] += ms; h->prof_n[sp.kind]++;
+    if (sp.kind == SPAN_STEP) h->prof_steps += sp.steps;
+    cudaEventDestroy(sp.a); cudaEventDestroy(sp.b);
+  }
+  h->spans.clear();
+  for (int k = 0; k < 3; ++k) { out[k] = h->prof_ms[k]; out[3 + k] = (double)h->prof_n[k]; h->prof_ms[k] = 0; h->prof_n[k] = 0; }
+  out[6] = (double)h->prof_steps; out[7] = 0;
+  h->prof_steps = 0;
+  return SOP_OK;
+}
+
+int sop_run(sop_handle *h, int64_t n_steps) {
+  if (!h || n_steps < 0) return fail(SOP_E_ARG, "bad handle or n_steps", h);
+  const int64_t nb = h->prm.nb_interval, plv = h->prm.pl_interval;
+  int64_t left = n_steps;
+  while (left > 0) {
+    if (h->plan.mode == 2) {
+      // one persistent launch runs up to the next pair-list boundary, re-filtering L2 inside
+      int64_t n = std::min<int64_t>(left, 1 << 20);
+      if (!h->S.static_l1) n = std::min<int64_t>(n, plv - (h->step % plv));
+      const bool l1_due = !h->S.static_l1 && (h->step + n) % plv == 0;
+      int rc = persistent_launch(h, (int)n, !l1_due);
+      if (rc) return rc;
+      h->cur ^= (int)(n & 1);
+      h->step += n; left -= n;
+      if (l1_due) { rc = rebuild_lists(h); if (rc) return rc; }
+      else if (h->step / nb * nb > h->l2_built_at) h->l2_built_at = h->step / nb * nb;
+    } else {
+      span_begin(h, SPAN_STEP, 1);
+      launch_step(h, false);
+      h->cur ^= 1; h->step++; left--;
+      if (!h->S.static_l1 && h->step % plv == 0) { int rc = launch_build_l1(h); if (rc) return rc; }
+      if (h->step % nb == 0) launch_filter(h);
+    }
+  }
+  span_close(h);
+  return check_launch(h, "sop_run");
+}
+
+int sop_sync(sop_handle *h) {
+  if (!h) return fail(SOP_E_ARG, "null handle");
+  return read_flags(h);
+}
+
+int sop_get_step(sop_handle *h, int64_t *step) {
+  if (!h || !step) return fail(SOP_E_ARG, "null argument", h);
+  *step = h->step;
+  return SOP_OK;
+}
+
+int sop_set_step(sop_handle *h, int64_t step) {
+  if (!h || step < 0) return fail(SOP_E_ARG, "bad step", h);
+  h->step = step; h->l1_built_at = step; h->l2_built_at = step;
+  return SOP_OK;
+}
+
+static int ensure_stage(sop_handle *h) {
+  if (h->stage) return SOP_OK;
+  CUDA_OK(cudaHostAlloc((void **)&h->stage, (size_t)h->S.n_inst * 16, cudaHostAllocDefault));
+  return SOP_OK;
+}
+
+int sop_get_coords(sop_handle *h, float *xyz_out) {
+  if (!h || !xyz_out) return fail(SOP_E_ARG, "null argument", h);
+  const int N = h->S.N, T = h->S.T;
+  int rc = ensure_stage(h);
+  if (rc) return rc;
+  CUDA_OK(cudaMemcpyAsync(h->stage, h->S.pos[h->cur], (size_t)N * T * 16, cudaMemcpyDeviceToHost, h->stream));
+  rc = read_flags(h);
+  for (int t = 0; t < T; ++t)
+    for (int ii = 0; ii < N; ++ii) {
+      const float4 &v = h->stage[(size_t)t * N + ii];
+      float *o = xyz_out + 3 * ((size_t)t * N + h->plan.perm[ii]);
+      o[0] = v.x; o[1] = v.y; o[2] = v.z;
+    }
+  return rc;
+}
+
+int sop_set_coords(sop_handle *h, const float *xyz) {
+  if (!h || !xyz) return fail(SOP_E_ARG, "null argument", h);
+  const int N = h->S.N, T = h->S.T;
+  int rc = ensure_stage(h);
+  if (rc) return rc;
+  CUDA_OK(cudaStreamSynchronize(h->stream));
+  for (int t = 0; t < T; ++t)
+    for (int ii = 0; ii < N; ++ii) {
+      const float *s = xyz + 3 * ((size_t)t * N + h->plan.perm[ii]);
+      float w; memcpy(&w, &h->tag[ii], 4);
+      h->stage[(size_t)t * N + ii] = make_float4(s[0], s[1], s[2], w);
+    }
+  CUDA_OK(cudaMemcpyAsync(h->S.pos[h->cur], h->stage, (size_t)N * T * 16, cudaMemcpyHostToDevice, h->stream));
+  if (h->S.carry) CUDA_OK(cudaMemsetAsync(h->S.carry, 0, (size_t)N * T * 16, h->stream));
+  rc = rebuild_lists(h);
+  if (rc) return rc;
+  return read_flags(h);
+}
+
+int sop_get_energies(sop_handle *h, double *e_out) {
+  if (!h || !e_out) return fail(SOP_E_ARG, "null argument", h);
+  const SysDev &S = h->S;
+  double *partial = (double *)(h->ws + h->plan.off_epart), *d_e = (double *)(h->ws + h->plan.off_eout);
+  dim3 grid((unsigned)h->plan.energy_blocks, (unsigned)S.T);
+  k_energy<<<grid, 256, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, partial);
+  k_energy_final<<<(S.T * 5 + 127) / 128, 128, 0, h->stream>>>(S.T, h->plan.energy_blocks, partial, d_e);
+  h->launches += 2;
+  int rc = check_launch(h, "energy");
+  if (rc) return rc;
+  CUDA_OK(cudaMemcpyAsync(e_out, d_e, (size_t)S.T * 6 * 8, cudaMemcpyDeviceToHost, h->stream));
+  rc = read_flags(h);
+  for (int t = 0; t < S.T; ++t) {
+    double *e = e_out + 6 * (size_t)t;
+    e[5] = e[0] + e[1] + e[2] + e[3] + e[4];
+  }
+  return rc;
+}
+
+int sop_get_forces(sop_handle *h, float *f_out) {
+  if (!h || !f_out) return fail(SOP_E_ARG, "null argument", h);
+  const int N = h->S.N, T = h->S.T;
+  int rc = ensure_stage(h);
+  if (rc) return rc;
+  launch_step(h, true);
+  rc = check_launch(h, "forces");
+  if (rc) return rc;
+  CUDA_OK(cudaMemcpyAsync(h->stage, h->S.force, (size_t)N * T * 16, cudaMemcpyDeviceToHost, h->stream));
+  rc = read_flags(h);
+  for (int t = 0; t < T; ++t)
+    for (int ii = 0; ii < N; ++ii) {
+      const float4 &v = h->stage[(size_t)t * N + ii];
+      float *o = f_out + 3 * ((size_t)t * N + h->plan.perm[ii]);
+      o[0] = v.x; o[1] = v.y; o[2] = v.z;
+    }
+  return rc;
+}
+
+int sop_get_lists(sop_handle *h, int32_t traj, int32_t level, int32_t *row_cnt, int32_t *idx, int32_t *cap_out,
+                  int64_t *built_at_step) {
+  if (!h || traj < 0 || traj >= h->S.T || (level != 1 && level != 2)) return fail(SOP_E_ARG, "bad argument", h);
+  const SysDev &S = h->S;
+  const int N = S.N;
+  const int cap = level == 1 ? S.cap_pl : S.cap_nb;
+  if (cap_out) *cap_out = cap;
+  if (built_at_step) *built_at_step = level == 1 ? h->l1_built_at : h->l2_built_at;
+  if (!row_cnt) return SOP_OK;
+  const size_t row0 = (level == 1 && S.static_l1) ? 0 : (size_t)traj * N;
+  const int *d_cnt = (level == 1 ? S.pl_cnt : S.nb_cnt) + row0;
+  const int *d_idx = (level == 1 ? S.pl_idx : S.nb_idx) + row0 * cap;
+  std::vector<int> cnt(N), rows;
+  CUDA_OK(cudaMemcpyAsync(cnt.data(), d_cnt, (size_t)N * 4, cudaMemcpyDeviceToHost, h->stream));
+  if (idx) {
+    rows.resize((size_t)N * cap);
+    CUDA_OK(cudaMemcpyAsync(rows.data(), d_idx, rows.size() * 4, cudaMemcpyDeviceToHost, h->stream));
+  }
+  int rc = read_flags(h);
+  for (int ii = 0; ii < N; ++ii) {
+    const int c = h->plan.perm[ii];
+    const int n = std::min(cnt[ii], cap);
+    row_cnt[c] = n;
+    if (idx) {
+      int *o = idx + (size_t)c * cap;
+      for (int q = 0; q < n; ++q) o[q] = h->plan.perm[rows[(size_t)ii * cap + q]];
+      std::sort(o, o + n);                       // rows ascending in the caller's index (reading R4)
+      for (int q = n; q < cap; ++q) o[q] = -1;
+    }
+  }
+  return rc;
+}
+
+int sop_device_coords(sop_handle *h, void **d_float4_out, int32_t *perm_out) {
+  if (!h || !d_float4_out) return fail(SOP_E_ARG, "null argument", h);
+  *d_float4_out = h->S.pos[h->cur];
+  if (perm_out) memcpy(perm_out, h->plan.perm.data(), (size_t)h->S.N * 4);
+  return SOP_OK;
+}
+
+int sop_get_config(sop_handle *h, int32_t out[9]) {
+  if (!h || !out) return fail(SOP_E_ARG, "null argument", h);
+  out[0] = h->plan.lanes; out[1] = h->plan.block; out[2] = h->plan.comp; out[3] = h->plan.mode;
+  out[4] = h->plan.reorder; out[5] = h->plan.cap_nb; out[6] = h->plan.cap_pl;
+  out[7] = (int32_t)(h->launches & 0xFFFFFFFFu); out[8] = (int32_t)(h->launches >> 32);
+  return SOP_OK;
+}
+
+}  // extern "C"

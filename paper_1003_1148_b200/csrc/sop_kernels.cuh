@@ -1,0 +1,350 @@
+// sop_kernels.cuh -- __global__ kernels of the SOP Langevin hot path (sm_100a).  See DESIGN.md "Kernels".
+#pragma once
+#include "sop_device.cuh"
+
+namespace sop {
+
+// ------------------------------------------------------------------------------------------------
+// a4-a9 fused: force + noise + integrate, one launch per step (the paper's single-kernel particle-based
+// organisation), G lanes per bead.  FORCES = true: the non-fused instantiation that writes the
+// deterministic force instead of moving the bead (sop_get_forces).
+// ------------------------------------------------------------------------------------------------
+template <int G, bool COMP, bool FORCES>
+__global__ void __launch_bounds__(1024) k_step(SysDev S, int cur, unsigned long long step) {
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int g = (int)(gid / G);
+  const int lane = (int)(gid % G);
+  const bool valid = g < S.n_inst;
+  const int gg = valid ? g : 0;
+  const int t = gg / S.N, i = gg - t * S.N;
+  const float4 *__restrict__ pos_t = S.pos[cur] + (size_t)t * S.N;
+  const float4 ri = __ldg(pos_t + i);
+  int flag = 0;
+  float3 f = internal_force<G, true>(S, pos_t, i, gg, lane, valid, ri, flag);
+  if (valid && lane == 0) {
+    const uint32_t tag = __float_as_uint(ri.w);
+    external_force(S, i, ri, tag, step, f.x, f.y, f.z, flag);
+    if (FORCES) {
+      S.force[gg] = make_float4(f.x, f.y, f.z, 0.f);
+    } else {
+      S.pos[cur ^ 1][gg] = langevin_update<COMP>(S, ri, tag, t, step, f.x, f.y, f.z, COMP ? S.carry + gg : nullptr, flag);
+    }
+  }
+  if (flag) atomicOr(S.flags, flag);
+}
+
+// a3: L2 neighbor-list filter (Alg. 3), one warp per bead instance.
+__global__ void __launch_bounds__(256) k_filter(SysDev S, int cur) {
+  const int w = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  const int lane = threadIdx.x & 31;
+  if (w >= S.n_inst) return;
+  const int t = w / S.N, i = w - t * S.N;
+  int flag = 0;
+  filter_row_warp<true>(S, S.pos[cur] + (size_t)t * S.N, i, w, lane, flag);
+  if (flag && lane == 0) atomicOr(S.flags, flag);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1: cell grid.  bbox -> grid parameters -> count -> scan -> fill -> per-cell sort (deterministic content).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int f2ord(float f) { int i = __float_as_int(f); return i >= 0 ? i : i ^ 0x7FFFFFFF; }
+__device__ __forceinline__ float ord2f(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7FFFFFFF); }
+
+__global__ void k_bbox_init(SysDev S) {
+  int q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q < S.T * 6) ((int *)S.bbox)[q] = (q % 6) < 3 ? 0x7FFFFFFF : (int)0x80000000;
+}
+
+__global__ void __launch_bounds__(256) k_bbox(SysDev S, int cur) {
+  // grid: (blocks, T)
+  const int t = blockIdx.y;
+  const float4 *pos_t = S.pos[cur] + (size_t)t * S.N;
+  float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < S.N; i += gridDim.x * blockDim.x) {
+    float4 r = __ldg(pos_t + i);
+    lo[0] = fminf(lo[0], r.x); lo[1] = fminf(lo[1], r.y); lo[2] = fminf(lo[2], r.z);
+    hi[0] = fmaxf(hi[0], r.x); hi[1] = fmaxf(hi[1], r.y); hi[2] = fmaxf(hi[2], r.z);
+  }
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+    for (int o = 16; o > 0; o >>= 1) {
+      lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+      hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+    }
+  if ((threadIdx.x & 31) == 0) {
+    int *bb = (int *)S.bbox + t * 6;
+    for (int a = 0; a < 3; ++a) { atomicMin(bb + a, f2ord(lo[a])); atomicMax(bb + 3 + a, f2ord(hi[a])); }
+  }
+}
+
+__global__ void k_grid_setup(SysDev S) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= S.T) return;
+  const int *bb = (const int *)S.bbox + t * 6;
+  float lo[3], ext[3];
+  for (int a = 0; a < 3; ++a) { lo[a] = ord2f(bb[a]); ext[a] = fmaxf(0.f, ord2f(bb[3 + a]) - lo[a]); }
+  float edge = S.cell_edge;
+  int n[3];
+  for (;;) {
+    long long tot = 1;
+    for (int a = 0; a < 3; ++a) { n[a] = (int)floorf(ext[a] / edge) + 1; tot *= n[a]; }
+    if (tot <= S.max_cells) break;
+    edge *= 1.25f;                       // cells may only grow: any edge >= cell_edge keeps the 27-cell scan complete
+  }
+  GridDev gd;
+  gd.ox = lo[0]; gd.oy = lo[1]; gd.oz = lo[2];
+  gd.inv_edge = 1.0f / edge;
+  gd.nx = n[0]; gd.ny = n[1]; gd.nz = n[2];
+  gd.ncell = n[0] * n[1] * n[2];
+  S.grid[t] = gd;
+}
+
+__device__ __forceinline__ int3 cell_coords(const GridDev &gd, const float4 &r) {
+  int cx = (int)floorf((r.x - gd.ox) * gd.inv_edge), cy = (int)floorf((r.y - gd.oy) * gd.inv_edge),
+      cz = (int)floorf((r.z - gd.oz) * gd.inv_edge);
+  cx = min(max(cx, 0), gd.nx - 1); cy = min(max(cy, 0), gd.ny - 1); cz = min(max(cz, 0), gd.nz - 1);
+  return make_int3(cx, cy, cz);
+}
+
+__global__ void __launch_bounds__(256) k_cell_count(SysDev S, int cur) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= S.n_inst) return;
+  const int t = g / S.N;
+  const GridDev gd = S.grid[t];
+  int3 c = cell_coords(gd, __ldg(S.pos[cur] + g));
+  int cell = (c.z * gd.ny + c.y) * gd.nx + c.x;
+  S.cell_of[g] = cell;
+  atomicAdd(&S.cell_cnt[(size_t)t * S.max_cells + cell], 1);
+}
+
+// exclusive scan of the cell counts of one trajectory by one block; zeroes the counts (they become fill cursors)
+__global__ void __launch_bounds__(1024) k_cell_scan(SysDev S) {
+  const int t = blockIdx.x;
+  const int ncell = S.grid[t].ncell;
+  int *cnt = S.cell_cnt + (size_t)t * S.max_cells;
+  int *start = S.cell_start + (size_t)t * (S.max_cells + 1);
+  __shared__ int warp_tot[32];
+  __shared__ int carry_s;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int base = 0; base < ncell; base += blockDim.x) {
+    int q = base + threadIdx.x;
+    int v = q < ncell ? cnt[q] : 0;
+    int inc = v;
+    for (int o = 1; o < 32; o <<= 1) { int n = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += n; }
+    if (lane == 31) warp_tot[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+      int w = lane < (blockDim.x >> 5) ? warp_tot[lane] : 0;
+      int winc = w;
+      for (int o = 1; o < 32; o <<= 1) { int n = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += n; }
+      warp_tot[lane] = winc - w;
+    }
+    __syncthreads();
+    int excl = carry_s + warp_tot[wid] + inc - v;
+    if (q < ncell) { start[q] = excl; cnt[q] = 0; }
+    __syncthreads();
+    if (threadIdx.x == blockDim.x - 1) carry_s = excl + v;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) start[ncell] = carry_s;
+}
+
+__global__ void __launch_bounds__(256) k_cell_fill(SysDev S) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= S.n_inst) return;
+  const int t = g / S.N, i = g - t * S.N;
+  const int cell = S.cell_of[g];
+  int slot = atomicAdd(&S.cell_cnt[(size_t)t * S.max_cells + cell], 1);
+  S.cell_bead[(size_t)t * S.N + S.cell_start[(size_t)t * (S.max_cells + 1) + cell] + slot] = i;
+}
+
+// One warp per cell: rank sort of the (distinct) bead indices so that the cell content, and with it every L1 row,
+// does not depend on the order in which the atomics of k_cell_fill were served.  cell_of is free by now: scratch.
+__global__ void __launch_bounds__(256) k_cell_sort(SysDev S) {
+  const int t = blockIdx.y;
+  const int ncell = S.grid[t].ncell;
+  const int lane = threadIdx.x & 31;
+  const int *start = S.cell_start + (size_t)t * (S.max_cells + 1);
+  int *bead = S.cell_bead + (size_t)t * S.N;
+  int *tmp = S.cell_of + (size_t)t * S.N;
+  for (int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < ncell; c += (gridDim.x * blockDim.x) >> 5) {
+    const int s = start[c], n = start[c + 1] - s;
+    for (int a = lane; a < n; a += 32) {
+      int v = bead[s + a], rank = 0;
+      for (int b = 0; b < n; ++b) rank += bead[s + b] < v;
+      tmp[s + rank] = v;
+    }
+    __syncwarp();
+    for (int a = lane; a < n; a += 32) bead[s + a] = tmp[s + a];
+    __syncwarp();
+  }
+}
+
+__device__ __forceinline__ bool is_excluded(const SysDev &S, int i, int j) {
+  int lo = __ldg(&S.excl_ptr[i]), hi = __ldg(&S.excl_ptr[i + 1]);
+  while (lo < hi) {
+    int mid = (lo + hi) >> 1;
+    int v = __ldg(&S.excl_idx[mid]);
+    if (v == j) return true;
+    if (v < j) lo = mid + 1; else hi = mid;
+  }
+  return false;
+}
+
+// a2: L1 pair-list build, one warp per bead instance: scan the 27 cells around the bead, keep j != i in the
+// non-native set with pred32(R_pl); ballot + prefix-popcount compaction (row order: cells z,y,x ascending, beads
+// ascending inside a cell -- deterministic; sop_get_lists returns rows sorted by the caller's index).
+__global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
+  const int w = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  const int lane = threadIdx.x & 31;
+  if (w >= S.n_inst) return;
+  const int t = w / S.N, i = w - t * S.N;
+  const float4 *__restrict__ pos_t = S.pos[cur] + (size_t)t * S.N;
+  const GridDev gd = S.grid[t];
+  const int *start = S.cell_start + (size_t)t * (S.max_cells + 1);
+  const int *bead = S.cell_bead + (size_t)t * S.N;
+  int *dst = S.pl_idx + (size_t)w * S.cap_pl;
+  const float4 ri = __ldg(pos_t + i);
+  const int3 c = cell_coords(gd, ri);
+  int n = 0;
+  for (int z = max(c.z - 1, 0); z <= min(c.z + 1, gd.nz - 1); ++z)
+    for (int y = max(c.y - 1, 0); y <= min(c.y + 1, gd.ny - 1); ++y) {
+      // the x-neighbours of a row of cells are contiguous in cell_bead: one segment per (z, y)
+      const int c0 = (z * gd.ny + y) * gd.nx + max(c.x - 1, 0), c1 = (z * gd.ny + y) * gd.nx + min(c.x + 1, gd.nx - 1);
+      const int s = start[c0], e = start[c1 + 1];
+      for (int base = s; base < e; base += 32) {
+        int q = base + lane;
+        int j = -1;
+        bool pass = false;
+        if (q < e) {
+          j = bead[q];
+          pass = j != i && pred32(ri, __ldg(pos_t + j), S.R_pl2) && !is_excluded(S, i, j);
+        }
+        unsigned m = __ballot_sync(0xffffffffu, pass);
+        if (pass) {
+          int slot = n + __popc(m & ((1u << lane) - 1u));
+          if (slot < S.cap_pl) dst[slot] = j;
+        }
+        n += __popc(m);
+      }
+    }
+  if (lane == 0) {
+    if (n > S.cap_pl) { atomicOr(S.flags, FLAG_PL_OVERFLOW); n = S.cap_pl; }
+    S.pl_cnt[w] = n;
+  }
+}
+
+// R_pl = +inf: the static all-pairs L1 (Table I's "non-native pairs"), one row per bead, shared.
+__global__ void __launch_bounds__(256) k_build_l1_static(SysDev S) {
+  const int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  const int lane = threadIdx.x & 31;
+  if (i >= S.N) return;
+  int *dst = S.pl_idx + (size_t)i * S.cap_pl;
+  int n = 0;
+  for (int base = 0; base < S.N; base += 32) {
+    int j = base + lane;
+    bool pass = j < S.N && j != i && !is_excluded(S, i, j);
+    unsigned m = __ballot_sync(0xffffffffu, pass);
+    if (pass) {
+      int slot = n + __popc(m & ((1u << lane) - 1u));
+      if (slot < S.cap_pl) dst[slot] = j;
+    }
+    n += __popc(m);
+  }
+  if (lane == 0) {
+    if (n > S.cap_pl) { atomicOr(S.flags, FLAG_PL_OVERFLOW); n = S.cap_pl; }
+    S.pl_cnt[i] = n;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a10: energies (Eq. (1) term by term, + external terms): fp32 pair terms, fp64 accumulation.
+// 8 lanes per bead; pair terms are visited from both ends and halved.  grid = (blocks, T);
+// partial[t][block][5] then k_energy_final sums the blocks in order (deterministic).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_energy(SysDev S, int cur, unsigned long long step, double *partial) {
+  constexpr int G = 8;
+  const int t = blockIdx.y;
+  const float4 *__restrict__ pos_t = S.pos[cur] + (size_t)t * S.N;
+  double e[5] = {0, 0, 0, 0, 0};
+  const int lane = threadIdx.x % G;
+  int flag = 0;
+  for (int i = (blockIdx.x * blockDim.x + threadIdx.x) / G; i < S.N; i += gridDim.x * blockDim.x / G) {
+    const int g = t * S.N + i;
+    const float4 ri = __ldg(pos_t + i);
+    for (int p = lane; p < S.cap_b; p += G) {
+      int2 b = __ldg(&S.bond_tab[(size_t)i * S.cap_b + p]);
+      if (b.x >= 0) {
+        float4 rj = __ldg(pos_t + b.x);
+        float dx = ri.x - rj.x, dy = ri.y - rj.y, dz = ri.z - rj.z;
+        bool bad; float ev;
+        fene_s(S, dx * dx + dy * dy + dz * dz, __int_as_float(b.y), bad, &ev);
+        if (bad) flag |= FLAG_FENE; else e[0] += 0.5 * (double)ev;
+      }
+    }
+    for (int q = __ldg(&S.nat_ptr[i]) + lane; q < __ldg(&S.nat_ptr[i + 1]); q += G) {
+      int2 b = __ldg(&S.nat_tab[q]);
+      float eps = S.nat_eps ? __ldg(&S.nat_eps[q]) : S.eps_native;
+      float4 rj = __ldg(pos_t + b.x);
+      float dx = ri.x - rj.x, dy = ri.y - rj.y, dz = ri.z - rj.z;
+      float ev;
+      native_s(dx * dx + dy * dy + dz * dz, __int_as_float(b.y), eps, &ev);
+      e[1] += 0.5 * (double)ev;
+    }
+    const int cnt = S.nb_cnt[g];
+    for (int p = lane; p < cnt; p += G) {
+      int j = S.nb_idx[(size_t)g * S.cap_nb + p];
+      float4 rj = __ldg(pos_t + j);
+      float dx = ri.x - rj.x, dy = ri.y - rj.y, dz = ri.z - rj.z;
+      float ev;
+      rep_s(S, dx * dx + dy * dy + dz * dz, &ev);
+      e[2] += 0.5 * (double)ev;
+    }
+    if (lane == 0) {
+      const uint32_t tag = __float_as_uint(ri.w);
+      if (S.has_pull && (tag & TAG_PULLED)) {
+        float vs = (float)((double)S.pull_v * (double)step);
+        float proj = ri.x * S.pull_nx + ri.y * S.pull_ny + ri.z * S.pull_nz - __ldg(&S.pull_adotn[i]);
+        float ext = vs - proj;
+        e[3] += (double)(0.5f * S.pull_k * ext * ext);
+      }
+      if (S.tip_on) {
+        float vs = (float)((double)S.tip_v * (double)step);
+        float dx = ri.x - (S.tip_cx + vs * S.tip_nx), dy = ri.y - (S.tip_cy + vs * S.tip_ny),
+              dz = ri.z - (S.tip_cz + vs * S.tip_nz);
+        float gap = sqrtf(dx * dx + dy * dy + dz * dz) - S.tip_R;
+        if (!(gap > 0.f)) flag |= FLAG_NONFINITE;
+        float ig = 1.0f / gap, ig2 = ig * ig;
+        e[4] += (double)(S.tip_eps * S.tip_sigma6 * ig2 * ig2 * ig2);
+      }
+    }
+  }
+  __shared__ double red[5][8];
+  const int wl = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    double v = e[k];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (wl == 0) red[k][wid] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 5) {
+    double v = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) v += red[threadIdx.x][w];
+    partial[((size_t)t * gridDim.x + blockIdx.x) * 5 + threadIdx.x] = v;
+  }
+  if (flag) atomicOr(S.flags, flag);
+}
+
+__global__ void k_energy_final(int T, int nblk, const double *partial, double *e_out) {
+  int q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= T * 5) return;
+  int t = q / 5, k = q % 5;
+  double v = 0;
+  for (int b = 0; b < nblk; ++b) v += partial[((size_t)t * nblk + b) * 5 + k];
+  e_out[t * 6 + k] = v;
+}
+
+}  // namespace sop

@@ -1,0 +1,316 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star):
+  lists        bit-exact at both levels (row counts and row contents, ascending caller index)
+  forces       max_i |F_gpu - F_cpu| <= 1e-4 * max_i |F_cpu|
+  coordinates  max |dr| <= 1e-3 A after 100 steps with the same Philox stream
+  energies     |dE| <= 1e-5 * sum of |terms|   (fp32 pair terms, fp64 accumulation; derived in DESIGN.md)
+"""
+import ctypes
+import math
+import os
+import subprocess
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import sopo
+from workloads import generators as gen
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def sop():
+    import paper_1003_1148_b200 as m
+    return m
+
+
+def perturbed32(w, amp, seed, n_traj=1):
+    r = np.random.default_rng(seed)
+    x = w.xyz[None].astype(np.float64) + amp * r.normal(size=(n_traj,) + w.xyz.shape)
+    return x.astype(np.float32)
+
+
+def rows_equal(a_cnt, a_idx, b_cnt, b_idx):
+    if not np.array_equal(a_cnt, b_cnt):
+        return False
+    m = int(a_cnt.max()) if len(a_cnt) else 0
+    A = np.where(np.arange(m)[None, :] < a_cnt[:, None], a_idx[:, :m], -1)
+    B = np.where(np.arange(m)[None, :] < b_cnt[:, None], b_idx[:, :m], -1)
+    return np.array_equal(A, B)
+
+
+def check_lists(s, o, x32, traj=0, builder=0):
+    """GPU lists (built from the fp32 snapshot x32 that both sides hold) == oracle lists, both levels."""
+    xd = x32.astype(np.float64)
+    for level in (1, 2):
+        gc, gi, _ = s.get_lists(level, traj)
+        oc, oi = o.build_lists(xd, level, builder, cap=gi.shape[1])
+        assert rows_equal(gc, gi, oc, oi), f"level {level} lists differ"
+
+
+def check_forces(s, o, x32, step=0):
+    f_gpu = s.get_forces()
+    for t in range(s.T):
+        o_t = o if o.T == 1 else None
+        _, f_cpu = o.eval_frozen(x32[t].astype(np.float64), step=step, traj=t if o.T > 1 else 0)
+        err = np.abs(f_gpu[t] - f_cpu).max()
+        assert err <= 1e-4 * np.abs(f_cpu).max(), (err, np.abs(f_cpu).max())
+
+
+def check_energies(e_gpu, e_cpu):
+    scale = np.abs(e_cpu[:, :5]).sum(axis=1, keepdims=True) + 1e-30
+    assert (np.abs(e_gpu - e_cpu) <= 1e-5 * scale).all(), (e_gpu, e_cpu)
+
+
+SMALL = [
+    ("tiny8", lambda: gen.tiny(8, 0), {}),
+    ("tiny100_pl20", lambda: gen.tiny(100, 2, R_pl=20.0), {}),
+    ("tiny257", lambda: gen.tiny(257, 3), {}),
+    ("two150_pl20", lambda: gen.two_chains(150, 1, R_pl=20.0), {}),
+    ("cfg0", gen.config0, {}),
+]
+VARIANTS = [dict(mode=1, lanes_per_bead=1), dict(mode=1, lanes_per_bead=8), dict(mode=1, lanes_per_bead=32),
+            dict(mode=2, lanes_per_bead=4), dict(mode=2, lanes_per_bead=16, reorder=1), dict(mode=1, reorder=1)]
+
+
+@pytest.mark.parametrize("name,make,over", SMALL, ids=[c[0] for c in SMALL])
+@pytest.mark.parametrize("var", VARIANTS, ids=lambda v: "-".join(f"{k}{v[k]}" for k in v))
+def test_small_lists_forces_energies_coords(name, make, over, var):
+    w = make()
+    s = sop().from_workload(w, **var, **over)
+    o = sopo.from_workload(w)
+    # native snapshot
+    x0 = w.xyz[None].copy()
+    check_lists(s, o, x0[0])
+    check_forces(s, o, x0)
+    check_energies(s.get_energies(), o.get_energies())
+    # perturbed snapshot: both sides rebuild their lists from the same fp32 coordinates
+    x1 = perturbed32(w, 0.3, 11)
+    s.set_coords(x1); o.set_coords(x1.astype(np.float64))
+    check_lists(s, o, x1[0])
+    check_forces(s, o, x1)
+    check_energies(s.get_energies(), o.get_energies())
+    # 100 steps from the native structure, same Philox stream
+    s.set_coords(x0); o.set_coords(x0.astype(np.float64))
+    s.step = 0; o.step = 0
+    s.run(100); o.run(100)
+    xg = s.get_coords(); xo = o.get_coords()
+    assert np.abs(xg - xo).max() <= 1e-3
+    assert s.step == 100
+    # list invariant: at step 100 both levels were rebuilt from the current coordinates
+    assert s.get_lists(2)[2] == 100
+    check_lists(s, o, xg[0])
+    check_energies(s.get_energies(), sopo_energies_at(o, xg))
+
+
+def sopo_energies_at(o, x32):
+    """oracle energies at the GPU's coordinates with lists rebuilt from them (so that V_rep sums the same pairs)"""
+    o2 = o
+    keep = o2.get_coords(); step = o2.step
+    o2.set_coords(x32.astype(np.float64))
+    e = o2.get_energies()
+    o2.set_coords(keep); o2.step = step
+    return e
+
+
+def test_run_split_variant_and_mode_independence():
+    w = gen.tiny(200, 5, R_pl=20.0)
+    ref = None
+    for var in (dict(mode=1, lanes_per_bead=4), dict(mode=2, lanes_per_bead=4)):
+        a = sop().from_workload(w, **var); a.run(130)
+        b = sop().from_workload(w, **var); b.run(7); b.run(93); b.run(30)
+        xa, xb = a.get_coords(), b.get_coords()
+        assert np.array_equal(xa, xb)                      # same variant: bit-identical however the run is split
+        for lv in (1, 2):
+            ca, ia, ata = a.get_lists(lv); cb, ib, atb = b.get_lists(lv)
+            assert rows_equal(ca, ia, cb, ib) and ata == atb
+        assert a.get_lists(1)[2] == 100 and a.get_lists(2)[2] == 130
+        if ref is None:
+            ref = xa
+        else:
+            assert np.array_equal(ref, xa)                 # per-step launches and the persistent kernel agree bit for bit
+    c = sop().from_workload(w, mode=1, lanes_per_bead=32, reorder=1); c.run(130)
+    assert np.abs(c.get_coords() - ref).max() < 1e-4       # other summation order: fp32 rounding only
+
+
+def test_checkpoint_resume_is_exact():
+    w = gen.tiny(128, 9, R_pl=20.0)
+    a = sop().from_workload(w, mode=2); a.run(300)
+    b = sop().from_workload(w, mode=2); b.run(200)
+    x = b.get_coords()
+    c = sop().from_workload(w, mode=2); c.set_coords(x); c.step = 200; c.run(100)
+    assert np.array_equal(a.get_coords(), c.get_coords())
+
+
+def test_batch_trajectories_and_sharding_offset():
+    w = gen.tiny(96, 4)
+    T = 5
+    s = sop().from_workload(w, n_traj=T, mode=2); s.run(100)
+    o = sopo.from_workload(w, n_traj=T); o.run(100)
+    xg, xo = s.get_coords(), o.get_coords()
+    assert np.abs(xg - xo).max() <= 1e-3
+    assert not np.array_equal(xg[0], xg[1])
+    for t in range(T):
+        gc, gi, _ = s.get_lists(2, t)
+        oc, oi = o.build_lists(xg[t].astype(np.float64), 2, cap=gi.shape[1])
+        assert rows_equal(gc, gi, oc, oi)
+    check_energies(s.get_energies(), sopo_energies_at(o, xg))
+    # a shard of the batch (trajectories 3..4 on another GPU) reproduces the unsharded batch bit for bit
+    from paper_1003_1148_b200 import shard_trajectories
+    off, n = shard_trajectories(T, 1, 2)
+    assert (off, n) == (3, 2)
+    sh = sop().from_workload(w, n_traj=n, mode=2, traj_offset=off); sh.run(100)
+    assert np.array_equal(sh.get_coords(), xg[off:off + n])
+
+
+def test_external_forces_pull_fixed_indenter_compensated():
+    w = gen.tiny(64, 8)
+    zmax = float(w.xyz[:, 2].max())
+    p = dict(w.params, fixed=[0, 5], pulled=[63, 20], pull_k=0.05, pull_v=1e-3, pull_dir=[0.6, 0.0, 0.8],
+             tip_on=1, tip_R=50.0, tip_eps=1.0, tip_sigma=3.8, tip_c0=[0.0, 0.0, zmax + 53.0],
+             tip_dir=[0.0, 0.0, -1.0], tip_v=1e-3)
+    for var in (dict(mode=1, compensated=2), dict(mode=2, compensated=1, lanes_per_bead=8)):
+        s = sop().Sop(w.xyz, w.bonds, w.native, p, **var)
+        o = sopo.Oracle(w.xyz, w.bonds, w.native, p)
+        s.step = 1000; o.step = 1000                         # the spring base and the tip have advanced
+        check_forces(s, o, w.xyz[None], step=1000)
+        check_energies(s.get_energies(), o.get_energies())
+        assert o.get_energies()[0, 3] > 0 and o.get_energies()[0, 4] > 0
+        s.run(100); o.run(100)
+        xg, xo = s.get_coords(), o.get_coords()
+        assert np.abs(xg - xo).max() <= 1e-3
+        assert np.array_equal(xg[0, 0], w.xyz[0]) and np.array_equal(xg[0, 5], w.xyz[5])   # fixed beads never move
+
+
+def test_compensated_update_at_large_coordinates():
+    """Reading R10: at |x| ~ 2700 A plain fp32 accumulation drifts past 1e-3 A in 100 steps; Kahan does not."""
+    w = gen.tiny(64, 10)
+    shift = np.array([0.0, 0.0, 2700.0], np.float32)
+    xyz = w.xyz + shift
+    o = sopo.Oracle(xyz, w.bonds, w.native, w.params); o.run(100)
+    s = sop().Sop(xyz, w.bonds, w.native, w.params, mode=2)     # compensated auto: on (max|coord| > 512)
+    assert s.config()["compensated"] == 1
+    s.run(100)
+    assert np.abs(s.get_coords() - o.get_coords()).max() <= 1e-3
+
+
+def test_error_flags():
+    m = sop()
+    w = gen.tiny(32, 1)
+    s = m.from_workload(w)
+    x = w.xyz[None].copy(); x[0, 10] += np.array([2.5, 0, 0], np.float32)       # bond 9-10 or 10-11 beyond R0
+    s.set_coords(x)
+    with pytest.raises(m.SopError) as ei:
+        s.get_forces()
+    assert ei.value.code == -4
+    with pytest.raises(m.SopError) as ei:
+        m.from_workload(w, cap_nb=4)                                             # rows overflow -> error, not truncation
+    assert ei.value.code == -3
+    with pytest.raises(m.SopError) as ei:
+        m.Sop(w.xyz, w.bonds, np.concatenate([w.native, w.bonds[:1]]), w.params)
+    assert ei.value.code == -1
+    with pytest.raises(m.SopError):
+        m.Sop(w.xyz, w.bonds, w.native, dict(w.params, pl_interval=15))
+
+
+def test_p5_free_diffusion_on_gpu():
+    N, n = 20000, 40
+    w = gen.free_beads(N, R_pl=20.0)
+    s = sop().from_workload(w, n_traj=2, mode=2)
+    x0 = s.get_coords().astype(np.float64)
+    s.run(n)
+    d = s.get_coords().astype(np.float64) - x0
+    kT, D = float(np.float32(0.6)), float(np.float32(2e-3))
+    var = 2 * kT * D * n
+    M = d.size
+    assert abs(d.mean()) < 5 * math.sqrt(var / M)
+    assert d.var() == pytest.approx(var, rel=5 * math.sqrt(2.0 / M) + 1e-4)
+    z = d / math.sqrt(var)
+    assert abs((z ** 4).mean() - 3.0) < 5 * math.sqrt(96.0 / M)
+    assert abs((z[..., 0] * z[..., 1]).mean()) < 5 / math.sqrt(2 * N)
+    assert abs((z[0] * z[1]).mean()) < 5 / math.sqrt(3 * N)
+
+
+def test_p6_device_philox_equals_curand_and_oracle():
+    src = os.path.join(HERE, "cuda", "philox_check.cu")
+    out = os.path.join(HERE, "cuda", "philox_check.so")
+    if not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src):
+        subprocess.check_call(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O2", "-std=c++17", "--shared",
+                               "-Xcompiler", "-fPIC", src, "-o", out])
+    L = ctypes.CDLL(out)
+    r = np.random.default_rng(2024)
+    n = 4096
+    ctr = r.integers(0, 2 ** 32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    key = r.integers(0, 2 ** 32, size=(n, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[:4] = [[0, 0, 0, 0], [0xFFFFFFFF] * 4, [0x243F6A88, 0x85A308D3, 0x13198A2E, 0x03707344], [1, 0, 0, 0]]
+    key[:4] = [[0, 0], [0xFFFFFFFF] * 2, [0xA4093822, 0x299F31D0], [0, 0]]
+    mine = np.zeros((n, 4), np.uint32); ref = np.zeros((n, 4), np.uint32); nor = np.zeros((n, 3), np.float32)
+    seed = 0x1234567890ABCDEF
+    assert L.philox_check(ctr.ctypes.data_as(ctypes.c_void_p), key.ctypes.data_as(ctypes.c_void_p), n,
+                          mine.ctypes.data_as(ctypes.c_void_p), ref.ctypes.data_as(ctypes.c_void_p),
+                          nor.ctypes.data_as(ctypes.c_void_p), ctypes.c_ulonglong(seed)) == 0
+    assert np.array_equal(mine, ref)                                   # product Philox == cuRAND device function
+    for q in range(64):
+        assert sopo.philox4x32_10(ctr[q], key[q]).tolist() == mine[q].tolist()      # == oracle Philox
+        step = int(ctr[q, 2]) | (int(ctr[q, 3]) << 32)
+        g = sopo.normals(seed, int(ctr[q, 0]), int(ctr[q, 1]), step)
+        assert np.abs(nor[q] - g).max() < 2e-5                         # fp32 Box-Muller with fast intrinsics
+
+
+# ---------------------------------------------------------------------------------------------- full-size configs
+def full_check(k, n_traj=None, steps=100, builder=1, sample_traj=(0,), **var):
+    w = gen.make_config(k)
+    T = w.n_traj if n_traj is None else n_traj
+    s = sop().from_workload(w, n_traj=T, **var)
+    o = sopo.from_workload(w, n_traj=T, list_builder=builder)
+    x0 = np.broadcast_to(w.xyz, (T,) + w.xyz.shape)
+    for t in sample_traj:
+        check_lists(s, o, w.xyz, traj=t, builder=builder)
+    f_gpu = s.get_forces(); f_cpu = o.get_forces()
+    assert np.abs(f_gpu - f_cpu).max() <= 1e-4 * np.abs(f_cpu).max()
+    check_energies(s.get_energies(), o.get_energies())
+    s.run(steps); o.run(steps)
+    xg, xo = s.get_coords(), o.get_coords()
+    err = np.abs(xg - xo).max()
+    assert err <= 1e-3, err
+    for t in sample_traj:
+        check_lists(s, o, xg[t], traj=t, builder=builder)
+    # forces and energies at the GPU's own step-100 coordinates
+    o.set_coords(xg.astype(np.float64)); o.step = steps
+    f_gpu = s.get_forces(); f_cpu = o.get_forces()
+    assert np.abs(f_gpu - f_cpu).max() <= 1e-4 * np.abs(f_cpu).max()
+    check_energies(s.get_energies(), o.get_energies())
+    return s
+
+
+def test_full_config1_batch():
+    full_check(1, n_traj=256, builder=0, sample_traj=(0, 137, 255), mode=2)
+
+
+def test_full_config1_batch_finite_pair_list():
+    w = gen.config1(R_pl=20.0)
+    T = 16
+    s = sop().from_workload(w, n_traj=T, mode=2)
+    o = sopo.from_workload(w, n_traj=T)
+    s.run(100); o.run(100)
+    xg = s.get_coords()
+    assert np.abs(xg - o.get_coords()).max() <= 1e-3
+    for t in (0, 15):
+        check_lists(s, o, xg[t], traj=t)
+
+
+def test_full_config2_fiber_pulled():
+    s = full_check(2, mode=2)
+    assert s.config()["compensated"] == 1
+
+
+def test_full_config3_shell_indented():
+    full_check(3, mode=2)
+    full_check(3, mode=1, steps=100)
+
+
+def test_full_config4_lattice():
+    full_check(4, mode=1)
