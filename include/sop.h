@@ -76,9 +76,13 @@ typedef struct {
   int32_t block_size;                /* 0 auto; threads per block of the step kernel (multiple of 32) */
   int32_t compensated;               /* 0 auto (on if max|coord| > 512 A), 1 on, 2 off: Kahan-compensated
                                         position update (keeps fp32 coordinates accurate at |x| ~ 10^3 A) */
-  int32_t mode;                      /* 0 auto, 1 one launch per step, 2 persistent multi-step kernel */
+  int32_t mode;                      /* 0 auto (3 when the chunk state fits shared memory, else 2), 1 one launch per
+                                        step, 2 persistent streaming kernel (grid barrier per step), 3 SM-resident
+                                        persistent kernel: a chunk of beads + halo + its L2 rows live in shared
+                                        memory, chunks exchange coordinates through stamped words in L2 */
   int32_t reorder;                   /* 0 auto, 1 sort beads by native position inside the library, 2 keep order;
                                         invisible at the boundary (all indices in and out are the caller's) */
+  int32_t chunk_beads;               /* mode 3: beads per chunk (one chunk per CTA); 0 auto */
   void *stream;                      /* cudaStream_t */
 } sop_params;
 
@@ -117,7 +121,7 @@ int sop_set_step(sop_handle *, int64_t step);       /* with sop_set_coords: exac
 /* Zero-copy view of the current coordinate layer: DEVICE float4 [T][N] in the library's internal bead order;
  * perm_out (HOST [N], may be NULL) receives the caller index of each internal slot. */
 int sop_device_coords(sop_handle *, void **d_float4_out, int32_t *perm_out);
-/* What the auto settings resolved to: lanes_per_bead, block_size, compensated(0/1), mode(1/2), reorder(0/1),
+/* What the auto settings resolved to: lanes_per_bead, block_size, compensated(0/1), mode(1/2/3), reorder(0/1),
  * cap_nb, cap_pl, kernel launches issued so far (lo, hi). */
 int sop_get_config(sop_handle *, int32_t out[9]);
 /* Kernel timing for the bench (CUDA events on the handle's stream around groups of launches of one kind).

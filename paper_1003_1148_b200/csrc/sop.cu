@@ -12,6 +12,7 @@
 
 #include "sop_kernels.cuh"
 #include "sop_persistent.cuh"
+#include "sop_resident.cuh"
 
 using namespace sop;
 
@@ -32,6 +33,12 @@ struct Plan {                     // everything that depends only on (topology, 
   size_t off_pos0, off_pos1, off_carry, off_force, off_bond, off_natptr, off_nattab, off_nateps, off_exclptr,
       off_exclidx, off_adotn, off_plcnt, off_plidx, off_nbcnt, off_nbidx, off_bbox, off_grid, off_cellof,
       off_cellcnt, off_cellstart, off_cellbead, off_flags, off_epart, off_eout, off_bar, total;
+  // mode 3 (SM-resident kernel): chunking, launch shape, shared-memory carve-up, workspace
+  bool res_ok = false;
+  std::string res_why;
+  int res_lanes = 1, res_block = 1024;
+  ResDev R;
+  size_t off_nhalo, off_hgid, off_plloc, off_natloc, off_bondloc, off_xch;
 };
 
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -61,6 +68,9 @@ struct sop_handle {
   int coop_block_size = 0;
   int num_sms = 0;
   unsigned *S_bar = nullptr;      // grid-barrier counter of the persistent kernel
+  ResDev R;                       // mode 3
+  const void *res_fn = nullptr;
+  uint32_t res_launch_id = 0;
   std::vector<uint32_t> tag;      // [N] host copy of the coordinate tags (internal order)
   float4 *stage = nullptr;        // pinned host staging buffer [T][N] for coordinate transfers
   // optional kernel timing (sop_set_profiling): event pairs around groups of launches of one kind
@@ -81,8 +91,9 @@ int fail(int code, const std::string &msg, sop_handle *h) {
 }
 
 // ---- host-side neighbour statistics of the native structure (sizing only; not on the hot path) ----------
-int max_neighbors(const std::vector<double> &x, int N, double R) {
-  if (!std::isfinite(R)) return N - 1;
+// fn(i, j) for every ordered pair i != j closer than R (cell list over the bounding box)
+template <class F>
+void visit_neighbors(const std::vector<double> &x, int N, double R, F fn) {
   double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
   for (int i = 0; i < N; ++i)
     for (int a = 0; a < 3; ++a) { lo[a] = std::min(lo[a], x[3 * i + a]); hi[a] = std::max(hi[a], x[3 * i + a]); }
@@ -98,22 +109,36 @@ int max_neighbors(const std::vector<double> &x, int N, double R) {
   std::vector<int> fill(start.begin(), start.end() - 1);
   for (int i = 0; i < N; ++i) order[fill[of[i]]++] = i;
   const double R2 = R * R;
-  int best = 0;
   for (int i = 0; i < N; ++i) {
-    int cx = cell(i, 0), cy = cell(i, 1), cz = cell(i, 2), cnt = 0;
+    int cx = cell(i, 0), cy = cell(i, 1), cz = cell(i, 2);
     for (int z = std::max(0, cz - 1); z <= std::min(n[2] - 1, cz + 1); ++z)
       for (int y = std::max(0, cy - 1); y <= std::min(n[1] - 1, cy + 1); ++y)
         for (int xx = std::max(0, cx - 1); xx <= std::min(n[0] - 1, cx + 1); ++xx) {
           int c = (z * n[1] + y) * n[0] + xx;
           for (int q = start[c]; q < start[c + 1]; ++q) {
             int j = order[q];
+            if (j == i) continue;
             double dx = x[3 * i] - x[3 * j], dy = x[3 * i + 1] - x[3 * j + 1], dz = x[3 * i + 2] - x[3 * j + 2];
-            cnt += (dx * dx + dy * dy + dz * dz < R2);
+            if (dx * dx + dy * dy + dz * dz < R2) fn(i, j);
           }
         }
-    best = std::max(best, cnt - 1);
   }
-  return best;
+}
+
+int max_neighbors(const std::vector<double> &x, int N, double R) {
+  if (!std::isfinite(R)) return N - 1;
+  std::vector<int> cnt(N, 0);
+  visit_neighbors(x, N, R, [&](int i, int) { cnt[i]++; });
+  return *std::max_element(cnt.begin(), cnt.end());
+}
+
+int device_sm_count() {
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
+    cudaGetLastError();
+    return 148;                       // B200; only reached without a device (sizing queries)
+  }
+  return n;
 }
 
 uint32_t part1by2(uint32_t v) {   // spread the low 10 bits of v
@@ -123,6 +148,69 @@ uint32_t part1by2(uint32_t v) {   // spread the low 10 bits of v
   v = (v | (v << 4)) & 0x030C30C3;
   v = (v | (v << 2)) & 0x09249249;
   return v;
+}
+
+// ---- mode 3 plan: chunks, lanes, halo capacity from the native structure, shared-memory carve-up ------------
+void plan_resident(const sop_params *p, const std::vector<double> &x, Plan &pl) {
+  const int N = pl.N, T = pl.T;
+  ResDev &R = pl.R;
+  memset(&R, 0, sizeof(R));
+  pl.res_ok = false;
+  const int sms = device_sm_count();
+  int C = 1;
+  if (!pl.static_l1) {
+    const int maxC = std::max(1, sms / T);
+    C = std::max(1, std::min(maxC, N / 192));
+  }
+  int chunk = (N + C - 1) / C;
+  if (p->chunk_beads > 0 && !pl.static_l1) chunk = std::min(N, (int)p->chunk_beads);
+  C = (N + chunk - 1) / chunk;
+  R.C = C; R.chunk = chunk;
+  R.implicit_l1 = pl.static_l1 ? 1 : 0;
+  R.nat_entries = (int)pl.n_nat_entries;
+  int G = p->lanes_per_bead;
+  if (G == 0) { G = 32; while (G > 1 && (long long)chunk * G > 1024) G >>= 1; }
+  pl.res_lanes = G;
+  int block = p->block_size > 0 ? p->block_size : (int)std::min<long long>(1024, ((long long)chunk * G + 31) / 32 * 32);
+  block = std::max(block, 32);
+  pl.res_block = block;
+  // halo capacity: beads of other chunks within 1.1 R_pl of a chunk's beads at the native structure, + 25 % + 64
+  int halo_cap = 32;
+  if (C > 1) {
+    std::vector<int> cnt(C, 0);
+    // chunk of a bead = internal index / chunk; distinct (chunk, outside bead) keys
+    std::vector<uint64_t> keys;
+    keys.reserve((size_t)N * 64);
+    visit_neighbors(x, N, (double)p->R_pl * 1.1, [&](int i, int j) {
+      const int ci = pl.iperm[i] / chunk, jj = pl.iperm[j];
+      if (jj / chunk != ci) keys.push_back(((uint64_t)ci << 32) | (uint32_t)jj);
+    });
+    std::sort(keys.begin(), keys.end());
+    keys.erase(std::unique(keys.begin(), keys.end()), keys.end());
+    for (uint64_t k : keys) cnt[(int)(k >> 32)]++;
+    const int worst = *std::max_element(cnt.begin(), cnt.end());
+    halo_cap = ((int)(worst * 1.25) + 64 + 31) / 32 * 32;
+  }
+  R.halo_cap = halo_cap;
+  const long long slots = (long long)chunk + halo_cap;
+  if (slots > 65535) { pl.res_why = "a chunk and its halo exceed 65535 slots"; return; }
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = (o + bytes + 15) / 16 * 16; return (int)at; };
+  R.off_pos = take(2 * (size_t)slots * 16);
+  R.off_g = take(G > 1 ? 2 * (size_t)chunk * 16 : 0);
+  R.off_carry = take(pl.comp ? (size_t)chunk * 16 : 0);
+  R.off_tag = take((size_t)chunk * 4);
+  if (G == 1) { R.nb_si = 1; R.nb_sp = (chunk + 31) / 32 * 32; R.off_nb = take((size_t)R.nb_sp * pl.cap_nb * 2); }
+  else { R.nb_si = pl.cap_nb + 2; R.nb_sp = 1; R.off_nb = take((size_t)chunk * R.nb_si * 2); }
+  R.off_cnt = take((size_t)chunk * 2);
+  R.off_active = take((size_t)halo_cap * 2);
+  R.off_bm = take((size_t)(halo_cap / 32 + 1) * 4);
+  R.off_sbm = take((size_t)(halo_cap / 32 + 1) * 4);
+  R.off_misc = take(64);
+  R.smem_bytes = (int)o;
+  if (o > 232448) { pl.res_why = "chunk state does not fit the 227 KB of shared memory of an SM"; return; }
+  if ((size_t)((N + 31) / 32) * 8 > 200000) { pl.res_why = "n_beads too large for the localise bitmap"; return; }
+  pl.res_ok = true;
 }
 
 int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int32_t T, Plan &pl) {
@@ -145,7 +233,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.comp = p->compensated == 1 || (p->compensated == 0 && maxabs > 512.0);
 
   // internal bead order: Morton order of 8 A cells of the native structure (gather locality), ties by index
-  pl.reorder = p->reorder == 1;
+  pl.reorder = p->reorder == 1 || (p->reorder == 0 && (p->mode == 0 || p->mode == 3));
   pl.perm.resize(N); pl.iperm.resize(N);
   for (int i = 0; i < N; ++i) pl.perm[i] = i;
   if (pl.reorder) {
@@ -211,8 +299,13 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.lanes = lanes;
   pl.block = p->block_size > 0 ? p->block_size : 256;
   if (pl.block % 32 || pl.block > 1024) return fail(SOP_E_ARG, "block_size must be a multiple of 32, <= 1024");
-  pl.mode = p->mode == 0 ? 1 : p->mode;
-  if (pl.mode != 1 && pl.mode != 2) return fail(SOP_E_ARG, "mode must be 0, 1 or 2");
+  if (p->mode < 0 || p->mode > 3) return fail(SOP_E_ARG, "mode must be 0, 1, 2 or 3");
+  pl.mode = p->mode;
+  if (pl.mode == 0 || pl.mode == 3) {
+    plan_resident(p, x, pl);
+    if (pl.mode == 3 && !pl.res_ok) return fail(SOP_E_ARG, "mode 3 is not possible here: " + pl.res_why);
+    pl.mode = pl.res_ok ? 3 : 2;
+  }
   pl.energy_blocks = (int)std::min<long long>(64, ((long long)N * 8 + 255) / 256);
 
   // workspace
@@ -241,6 +334,16 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.off_epart = take((size_t)T * pl.energy_blocks * 5 * 8);
   pl.off_eout = take((size_t)T * 6 * 8);
   pl.off_bar = take(256);
+  if (pl.mode == 3) {
+    const ResDev &R = pl.R;
+    const bool multi = R.C > 1;
+    pl.off_nhalo = take((size_t)T * R.C * 4);
+    pl.off_hgid = take((size_t)T * R.C * R.halo_cap * 4);
+    pl.off_plloc = take(R.implicit_l1 ? 0 : I * pl.cap_pl * 2);
+    pl.off_natloc = take(multi ? (size_t)T * pl.n_nat_entries * 2 : 0);
+    pl.off_bondloc = take(multi ? I * pl.cap_b * 2 : 0);
+    pl.off_xch = take(multi ? 2 * I * 32 : 0);
+  }
   pl.total = o;
   return SOP_OK;
 }
@@ -339,6 +442,7 @@ int read_flags(sop_handle *h) {
   if (flags & FLAG_NONFINITE) return fail(SOP_E_NONFINITE, "non-finite coordinate or bead inside the indenter", h);
   if (flags & FLAG_FENE) return fail(SOP_E_FENE, "a bond reached |r - r0| >= R0", h);
   if (flags & FLAG_PL_OVERFLOW) return fail(SOP_E_LIST_OVERFLOW, "pair-list row exceeded cap_pl", h);
+  if (flags & FLAG_SLOT_OVERFLOW) return fail(SOP_E_LIST_OVERFLOW, "the halo of a chunk exceeded its slot capacity (mode 3)", h);
   return fail(SOP_E_LIST_OVERFLOW, "neighbor-list row exceeded cap_nb", h);
 }
 
@@ -390,9 +494,73 @@ int persistent_launch(sop_handle *h, int n, bool filter_last) {
   return SOP_OK;
 }
 
+template <int G, bool COMP>
+const void *resident_fn() { return (const void *)k_resident<G, COMP>; }
+
+const void *resident_kernel(int lanes, bool comp) {
+  switch (lanes) {
+    case 1: return comp ? resident_fn<1, true>() : resident_fn<1, false>();
+    case 2: return comp ? resident_fn<2, true>() : resident_fn<2, false>();
+    case 4: return comp ? resident_fn<4, true>() : resident_fn<4, false>();
+    case 8: return comp ? resident_fn<8, true>() : resident_fn<8, false>();
+    case 16: return comp ? resident_fn<16, true>() : resident_fn<16, false>();
+    default: return comp ? resident_fn<32, true>() : resident_fn<32, false>();
+  }
+}
+
+int resident_prepare(sop_handle *h) {
+  const Plan &pl = h->plan;
+  h->R = pl.R;
+  ResDev &R = h->R;
+  char *w = h->ws;
+  R.n_halo = (int *)(w + pl.off_nhalo); R.halo_gid = (int *)(w + pl.off_hgid);
+  R.pl_loc = (unsigned short *)(w + pl.off_plloc); R.nat_loc = (unsigned short *)(w + pl.off_natloc);
+  R.bond_loc = (unsigned short *)(w + pl.off_bondloc); R.xch = (uint4 *)(w + pl.off_xch);
+  h->res_fn = resident_kernel(pl.res_lanes, pl.comp);
+  CUDA_OK(cudaFuncSetAttribute(h->res_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, R.smem_bytes));
+  const int loc_smem = ((h->S.N + 31) / 32) * 8;
+  CUDA_OK(cudaFuncSetAttribute((const void *)k_localise, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(loc_smem, 1024)));
+  int occ = 0;
+  CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->res_fn, pl.res_block, R.smem_bytes));
+  if (occ < 1) return fail(SOP_E_CUDA, "resident kernel does not fit on an SM", h);
+  if (R.C > 1) {
+    int coop = 0, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    if (!coop || (long long)h->S.T * R.C > (long long)occ * h->num_sms)
+      return fail(SOP_E_CUDA, "the chunks of mode 3 cannot all be co-resident on this device", h);
+    CUDA_OK(cudaMemsetAsync(R.xch, 0, 2 * (size_t)h->S.n_inst * 32, h->stream));
+  }
+  CUDA_OK(cudaMemsetAsync(R.n_halo, 0, (size_t)h->S.T * R.C * 4, h->stream));
+  return SOP_OK;
+}
+
+int resident_launch(sop_handle *h, int n, bool filter_last) {
+  span_close(h);
+  span_begin(h, SPAN_STEP, n);
+  SysDev S = h->S;
+  ResDev R = h->R;
+  int cur = h->cur;
+  unsigned long long step0 = (unsigned long long)h->step;
+  int nb = h->prm.nb_interval, fl = filter_last ? 1 : 0;
+  h->res_launch_id++;
+  uint32_t stamp0 = ((h->res_launch_id & 0xFFFu) << 20) | 1u;     // never 0, never the previous launch's stamps
+  void *args[] = {&S, &R, &cur, &step0, &n, &nb, &fl, &stamp0};
+  const dim3 grid((unsigned)(S.T * R.C)), block((unsigned)h->plan.res_block);
+  if (R.C > 1) CUDA_OK(cudaLaunchCooperativeKernel(h->res_fn, grid, block, args, (size_t)R.smem_bytes, h->stream));
+  else CUDA_OK(cudaLaunchKernel(h->res_fn, grid, block, args, (size_t)R.smem_bytes, h->stream));
+  h->launches++;
+  return SOP_OK;
+}
+
 int rebuild_lists(sop_handle *h) {
   int rc = launch_build_l1(h);
   if (rc) return rc;
+  if (h->plan.mode == 3 && !h->R.implicit_l1) {
+    const int loc_smem = ((h->S.N + 31) / 32) * 8;
+    k_localise<<<(unsigned)(h->S.T * h->R.C), 512, loc_smem, h->stream>>>(h->S, h->R);
+    h->launches++;
+  }
   launch_filter(h);
   span_close(h);
   return check_launch(h, "list rebuild");
@@ -574,6 +742,11 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
     if (rc) { std::string m = g_last_error; delete h; return fail(rc, m); }
   }
 
+  if (pl.mode == 3) {
+    rc = resident_prepare(h);
+    if (rc) { std::string m = g_last_error; delete h; return fail(rc, m); }
+  }
+
   h->cur = 0; h->step = 0;
   rc = rebuild_lists(h);
   if (!rc) rc = read_flags(h);
@@ -622,14 +795,14 @@ int sop_run(sop_handle *h, int64_t n_steps) {
   const int64_t nb = h->prm.nb_interval, plv = h->prm.pl_interval;
   int64_t left = n_steps;
   while (left > 0) {
-    if (h->plan.mode == 2) {
+    if (h->plan.mode >= 2) {
       // one persistent launch runs up to the next pair-list boundary, re-filtering L2 inside
-      int64_t n = std::min<int64_t>(left, 1 << 20);
+      int64_t n = std::min<int64_t>(left, (1 << 20) - 2);
       if (!h->S.static_l1) n = std::min<int64_t>(n, plv - (h->step % plv));
       const bool l1_due = !h->S.static_l1 && (h->step + n) % plv == 0;
-      int rc = persistent_launch(h, (int)n, !l1_due);
+      int rc = h->plan.mode == 3 ? resident_launch(h, (int)n, !l1_due) : persistent_launch(h, (int)n, !l1_due);
       if (rc) return rc;
-      h->cur ^= (int)(n & 1);
+      if (h->plan.mode == 2) h->cur ^= (int)(n & 1);      // mode 3 writes the final layer back in place
       h->step += n; left -= n;
       if (l1_due) { rc = rebuild_lists(h); if (rc) return rc; }
       else if (h->step / nb * nb > h->l2_built_at) h->l2_built_at = h->step / nb * nb;
@@ -783,7 +956,7 @@ int sop_device_coords(sop_handle *h, void **d_float4_out, int32_t *perm_out) {
 
 int sop_get_config(sop_handle *h, int32_t out[9]) {
   if (!h || !out) return fail(SOP_E_ARG, "null argument", h);
-  out[0] = h->plan.lanes; out[1] = h->plan.block; out[2] = h->plan.comp; out[3] = h->plan.mode;
+  out[0] = h->plan.mode == 3 ? h->plan.res_lanes : h->plan.lanes; out[1] = h->plan.mode == 3 ? h->plan.res_block : h->plan.block; out[2] = h->plan.comp; out[3] = h->plan.mode;
   out[4] = h->plan.reorder; out[5] = h->plan.cap_nb; out[6] = h->plan.cap_pl;
   out[7] = (int32_t)(h->launches & 0xFFFFFFFFu); out[8] = (int32_t)(h->launches >> 32);
   return SOP_OK;

@@ -232,13 +232,10 @@ __device__ __forceinline__ void external_force(const SysDev &S, int i, const flo
   }
 }
 
-// a8 + a9: noise and the position update of Alg. 7 line 5, optionally Kahan-compensated (R10).
+// a9: the position update of Alg. 7 line 5 given the three normals, optionally Kahan-compensated (R10).
 template <bool COMP>
-__device__ __forceinline__ float4 langevin_update(const SysDev &S, const float4 &ri, uint32_t tag, int t,
-                                                  unsigned long long step, float fx, float fy, float fz,
-                                                  float4 *carry_slot, int &flag) {
-  if (tag & TAG_FIXED) return ri;                                     // fixed beads are copied unchanged
-  float3 gn = gaussian3(S, tag & TAG_ID_MASK, (uint32_t)(S.traj_offset + t), step);
+__device__ __forceinline__ float4 langevin_apply(const SysDev &S, const float4 &ri, const float3 &gn, float fx, float fy,
+                                                 float fz, float4 *carry_slot, int &flag) {
   float dx = S.D * fx + S.amp * gn.x, dy = S.D * fy + S.amp * gn.y, dz = S.D * fz + S.amp * gn.z;
   float4 out;
   if (COMP) {
@@ -255,6 +252,16 @@ __device__ __forceinline__ float4 langevin_update(const SysDev &S, const float4 
   out.w = ri.w;
   if (!isfinite(out.x + out.y + out.z)) flag |= FLAG_NONFINITE;
   return out;
+}
+
+// a8 + a9: noise and the position update.
+template <bool COMP>
+__device__ __forceinline__ float4 langevin_update(const SysDev &S, const float4 &ri, uint32_t tag, int t,
+                                                  unsigned long long step, float fx, float fy, float fz,
+                                                  float4 *carry_slot, int &flag) {
+  if (tag & TAG_FIXED) return ri;                                     // fixed beads are copied unchanged
+  float3 gn = gaussian3(S, tag & TAG_ID_MASK, (uint32_t)(S.traj_offset + t), step);
+  return langevin_apply<COMP>(S, ri, gn, fx, fy, fz, carry_slot, flag);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -73,7 +73,9 @@ SMALL = [
     ("cfg0", gen.config0, {}),
 ]
 VARIANTS = [dict(mode=1, lanes_per_bead=1), dict(mode=1, lanes_per_bead=8), dict(mode=1, lanes_per_bead=32),
-            dict(mode=2, lanes_per_bead=4), dict(mode=2, lanes_per_bead=16, reorder=1), dict(mode=1, reorder=1)]
+            dict(mode=2, lanes_per_bead=4), dict(mode=2, lanes_per_bead=16, reorder=1), dict(mode=1, reorder=1),
+            dict(mode=3), dict(mode=3, chunk_beads=40, lanes_per_bead=4), dict(mode=3, chunk_beads=64, lanes_per_bead=1),
+            dict(mode=3, chunk_beads=33, lanes_per_bead=16, compensated=1)]
 
 
 @pytest.mark.parametrize("name,make,over", SMALL, ids=[c[0] for c in SMALL])
@@ -134,21 +136,36 @@ def test_run_split_variant_and_mode_independence():
             assert np.array_equal(ref, xa)                 # per-step launches and the persistent kernel agree bit for bit
     c = sop().from_workload(w, mode=1, lanes_per_bead=32, reorder=1); c.run(130)
     assert np.abs(c.get_coords() - ref).max() < 1e-4       # other summation order: fp32 rounding only
+    # the SM-resident kernel: bit-identical however the run is split and whatever else ran before on the exchange
+    # buffer; against the streaming kernels only the rounding of the pair terms differs
+    for var in (dict(mode=3), dict(mode=3, chunk_beads=48, lanes_per_bead=8)):
+        a = sop().from_workload(w, **var); a.run(130)
+        b = sop().from_workload(w, **var); b.run(7); b.run(93); b.run(1); b.run(29)
+        assert a.config()["mode"] == 3
+        assert np.array_equal(a.get_coords(), b.get_coords())
+        for lv in (1, 2):
+            ca, ia, ata = a.get_lists(lv); cb, ib, atb = b.get_lists(lv)
+            assert rows_equal(ca, ia, cb, ib) and ata == atb
+        assert a.get_lists(1)[2] == 100 and a.get_lists(2)[2] == 130
+        assert np.abs(a.get_coords() - ref).max() < 1e-4
 
 
-def test_checkpoint_resume_is_exact():
+@pytest.mark.parametrize("var", [dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=40)], ids=str)
+def test_checkpoint_resume_is_exact(var):
     w = gen.tiny(128, 9, R_pl=20.0)
-    a = sop().from_workload(w, mode=2); a.run(300)
-    b = sop().from_workload(w, mode=2); b.run(200)
+    a = sop().from_workload(w, **var); a.run(300)
+    b = sop().from_workload(w, **var); b.run(200)
     x = b.get_coords()
-    c = sop().from_workload(w, mode=2); c.set_coords(x); c.step = 200; c.run(100)
+    c = sop().from_workload(w, **var); c.set_coords(x); c.step = 200; c.run(100)
     assert np.array_equal(a.get_coords(), c.get_coords())
 
 
-def test_batch_trajectories_and_sharding_offset():
-    w = gen.tiny(96, 4)
+@pytest.mark.parametrize("var", [dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=32, R_pl=20.0)], ids=str)
+def test_batch_trajectories_and_sharding_offset(var):
+    var = dict(var)
+    w = gen.tiny(96, 4, **({"R_pl": var.pop("R_pl")} if "R_pl" in var else {}))
     T = 5
-    s = sop().from_workload(w, n_traj=T, mode=2); s.run(100)
+    s = sop().from_workload(w, n_traj=T, **var); s.run(100)
     o = sopo.from_workload(w, n_traj=T); o.run(100)
     xg, xo = s.get_coords(), o.get_coords()
     assert np.abs(xg - xo).max() <= 1e-3
@@ -162,7 +179,7 @@ def test_batch_trajectories_and_sharding_offset():
     from paper_1003_1148_b200 import shard_trajectories
     off, n = shard_trajectories(T, 1, 2)
     assert (off, n) == (3, 2)
-    sh = sop().from_workload(w, n_traj=n, mode=2, traj_offset=off); sh.run(100)
+    sh = sop().from_workload(w, n_traj=n, traj_offset=off, **var); sh.run(100)
     assert np.array_equal(sh.get_coords(), xg[off:off + n])
 
 
@@ -172,7 +189,11 @@ def test_external_forces_pull_fixed_indenter_compensated():
     p = dict(w.params, fixed=[0, 5], pulled=[63, 20], pull_k=0.05, pull_v=1e-3, pull_dir=[0.6, 0.0, 0.8],
              tip_on=1, tip_R=50.0, tip_eps=1.0, tip_sigma=3.8, tip_c0=[0.0, 0.0, zmax + 53.0],
              tip_dir=[0.0, 0.0, -1.0], tip_v=1e-3)
-    for var in (dict(mode=1, compensated=2), dict(mode=2, compensated=1, lanes_per_bead=8)):
+    for var in (dict(mode=1, compensated=2), dict(mode=2, compensated=1, lanes_per_bead=8), dict(mode=3),
+                dict(mode=3, compensated=1, lanes_per_bead=8, chunk_beads=24, R_pl=20.0)):
+        var = dict(var)
+        if "R_pl" in var:
+            p = dict(p, R_pl=var.pop("R_pl"), pl_interval=100)
         s = sop().Sop(w.xyz, w.bonds, w.native, p, **var)
         o = sopo.Oracle(w.xyz, w.bonds, w.native, p)
         s.step = 1000; o.step = 1000                         # the spring base and the tip have advanced
@@ -286,14 +307,17 @@ def full_check(k, n_traj=None, steps=100, builder=1, sample_traj=(0,), **var):
     return s
 
 
-def test_full_config1_batch():
-    full_check(1, n_traj=256, builder=0, sample_traj=(0, 137, 255), mode=2)
+@pytest.mark.parametrize("mode", [2, 3])
+def test_full_config1_batch(mode):
+    s = full_check(1, n_traj=256, builder=0, sample_traj=(0, 137, 255), mode=mode)
+    assert s.config()["mode"] == mode
 
 
 def test_full_config1_batch_finite_pair_list():
     w = gen.config1(R_pl=20.0)
     T = 16
-    s = sop().from_workload(w, n_traj=T, mode=2)
+    s = sop().from_workload(w, n_traj=T, mode=0)
+    assert s.config()["mode"] == 3
     o = sopo.from_workload(w, n_traj=T)
     s.run(100); o.run(100)
     xg = s.get_coords()
@@ -302,15 +326,18 @@ def test_full_config1_batch_finite_pair_list():
         check_lists(s, o, xg[t], traj=t)
 
 
-def test_full_config2_fiber_pulled():
-    s = full_check(2, mode=2)
-    assert s.config()["compensated"] == 1
+@pytest.mark.parametrize("mode", [2, 3])
+def test_full_config2_fiber_pulled(mode):
+    s = full_check(2, mode=mode)
+    assert s.config()["compensated"] == 1 and s.config()["mode"] == mode
 
 
-def test_full_config3_shell_indented():
-    full_check(3, mode=2)
-    full_check(3, mode=1, steps=100)
+@pytest.mark.parametrize("mode", [1, 2, 3])
+def test_full_config3_shell_indented(mode):
+    s = full_check(3, mode=mode)
+    assert s.config()["mode"] == mode
 
 
-def test_full_config4_lattice():
-    full_check(4, mode=1)
+@pytest.mark.parametrize("mode", [0, 1])
+def test_full_config4_lattice(mode):
+    full_check(4, mode=mode)
