@@ -203,8 +203,8 @@ def measure(w, T, traj_offset, block, K, W, clocks_index=None, e2e=True, overrid
     # force+integrate kernel alone (its own event spans inside the library, on the same stream)
     if prof["langevin_steps"] > 0 and prof["step_ms"] > 0:
         us_fi = prof["step_ms"] * 1e3 / prof["langevin_steps"]
-        n_filters_inside = prof["langevin_steps"] // w.params["nb_interval"] if cfg["mode"] == 2 else 0
-        bytes_per_launch_step = N * T * (ab["B_fi"] + (ab["B_filter"] / w.params["nb_interval"] if cfg["mode"] == 2 else 0.0))
+        n_filters_inside = prof["langevin_steps"] // w.params["nb_interval"] if cfg["mode"] >= 2 else 0
+        bytes_per_launch_step = N * T * (ab["B_fi"] + (ab["B_filter"] / w.params["nb_interval"] if cfg["mode"] >= 2 else 0.0))
         res["step_kernel"] = {"us_per_langevin_step": us_fi, "achieved_gbs": bytes_per_launch_step / (us_fi * 1e-6) / 1e9,
                               "includes_l2_filter": bool(n_filters_inside), "spans": prof["step_spans"]}
     if sampler:
