@@ -32,7 +32,7 @@ struct Plan {                     // everything that depends only on (topology, 
   // workspace offsets
   size_t off_pos0, off_pos1, off_carry, off_force, off_bond, off_natptr, off_nattab, off_nateps, off_exclptr,
       off_exclidx, off_adotn, off_plcnt, off_plidx, off_nbcnt, off_nbidx, off_bbox, off_grid, off_cellof,
-      off_cellcnt, off_cellstart, off_cellbead, off_flags, off_epart, off_eout, off_bar, total;
+      off_cellcnt, off_cellstart, off_cellbead, off_cellpos, off_flags, off_epart, off_eout, off_bar, total;
   // mode 3 (SM-resident kernel): chunking, launch shape, shared-memory carve-up, workspace
   bool res_ok = false;
   std::string res_why;
@@ -151,7 +151,7 @@ uint32_t part1by2(uint32_t v) {   // spread the low 10 bits of v
 }
 
 // ---- mode 3 plan: chunks, lanes, halo capacity from the native structure, shared-memory carve-up ------------
-void plan_resident(const sop_params *p, const std::vector<double> &x, Plan &pl) {
+void plan_resident(const sop_topology *tp, const sop_params *p, const std::vector<double> &x, Plan &pl) {
   const int N = pl.N, T = pl.T;
   ResDev &R = pl.R;
   memset(&R, 0, sizeof(R));
@@ -172,19 +172,21 @@ void plan_resident(const sop_params *p, const std::vector<double> &x, Plan &pl) 
   if (G == 0) { G = 32; while (G > 1 && (long long)chunk * G > 1024) G >>= 1; }
   pl.res_lanes = G;
   int block = p->block_size > 0 ? p->block_size : (int)std::min<long long>(1024, ((long long)chunk * G + 31) / 32 * 32);
-  block = std::max(block, 32);
-  pl.res_block = block;
+  pl.res_block = std::max(32, std::min(1024, block));
   // halo capacity: beads of other chunks within 1.1 R_pl of a chunk's beads at the native structure, + 25 % + 64
-  int halo_cap = 32;
+  int halo_cap = 32, pl_want = 0;
   if (C > 1) {
     std::vector<int> cnt(C, 0);
+    std::vector<long long> l1_entries(C, 0);
     // chunk of a bead = internal index / chunk; distinct (chunk, outside bead) keys
     std::vector<uint64_t> keys;
     keys.reserve((size_t)N * 64);
     visit_neighbors(x, N, (double)p->R_pl * 1.1, [&](int i, int j) {
       const int ci = pl.iperm[i] / chunk, jj = pl.iperm[j];
+      l1_entries[ci]++;
       if (jj / chunk != ci) keys.push_back(((uint64_t)ci << 32) | (uint32_t)jj);
     });
+    pl_want = (int)std::min<long long>(1 << 20, *std::max_element(l1_entries.begin(), l1_entries.end()) + chunk + 64);
     std::sort(keys.begin(), keys.end());
     keys.erase(std::unique(keys.begin(), keys.end()), keys.end());
     for (uint64_t k : keys) cnt[(int)(k >> 32)]++;
@@ -194,20 +196,46 @@ void plan_resident(const sop_params *p, const std::vector<double> &x, Plan &pl) 
   R.halo_cap = halo_cap;
   const long long slots = (long long)chunk + halo_cap;
   if (slots > 65535) { pl.res_why = "a chunk and its halo exceed 65535 slots"; return; }
+  // native entries per chunk (internal order)
+  {
+    std::vector<int> per(C, 0);
+    for (int c2 = 0; c2 < tp->n_native; ++c2) {
+      per[pl.iperm[tp->native[2 * c2]] / chunk]++;
+      per[pl.iperm[tp->native[2 * c2 + 1]] / chunk]++;
+    }
+    R.nat_cap = std::max(1, *std::max_element(per.begin(), per.end()));
+  }
+  R.nb_si = pl.cap_nb + 2;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = (o + bytes + 15) / 16 * 16; return (int)at; };
-  R.off_pos = take(2 * (size_t)slots * 16);
-  R.off_g = take(G > 1 ? 2 * (size_t)chunk * 16 : 0);
-  R.off_carry = take(pl.comp ? (size_t)chunk * 16 : 0);
-  R.off_tag = take((size_t)chunk * 4);
-  if (G == 1) { R.nb_si = 1; R.nb_sp = (chunk + 31) / 32 * 32; R.off_nb = take((size_t)R.nb_sp * pl.cap_nb * 2); }
-  else { R.nb_si = pl.cap_nb + 2; R.nb_sp = 1; R.off_nb = take((size_t)chunk * R.nb_si * 2); }
-  R.off_cnt = take((size_t)chunk * 2);
-  R.off_active = take((size_t)halo_cap * 2);
-  R.off_bm = take((size_t)(halo_cap / 32 + 1) * 4);
-  R.off_sbm = take((size_t)(halo_cap / 32 + 1) * 4);
-  R.off_misc = take(64);
-  R.smem_bytes = (int)o;
+  auto carve = [&](bool nat_smem, int pl_cap) {
+    o = 0;
+    R.nat_smem = nat_smem ? 1 : 0;
+    R.pl_cap = pl_cap;
+    R.off_pos = take(2 * (size_t)(slots + 1) * 16);
+    R.off_g = take(G > 1 ? 2 * (size_t)chunk * 16 : 0);
+    R.off_carry = take(pl.comp ? (size_t)chunk * 16 : 0);
+    R.off_tag = take((size_t)chunk * 4);
+    R.off_facc = take((size_t)chunk * 16);
+    R.off_nb = take((size_t)chunk * R.nb_si * 2);
+    R.off_cnt = take((size_t)chunk * 2);
+    R.off_rofs = take(((size_t)chunk + 1) * 4);
+    R.off_plcnt = take((size_t)chunk * 2);
+    R.off_plofs = take(((size_t)chunk + 1) * 4);
+    R.off_pl = take((size_t)pl_cap * 2);
+    R.off_natq = take(((size_t)chunk + 1) * 4);
+    R.off_nat = take(nat_smem ? (size_t)R.nat_cap * 8 : 0);
+    R.off_bond = take((size_t)chunk * pl.cap_b * 8);
+    R.off_active = take((size_t)halo_cap * 2);
+    R.off_bm = take((size_t)(halo_cap / 32 + 1) * 4);
+    R.off_sbm = take((size_t)(halo_cap / 32 + 1) * 4);
+    R.off_misc = take(64);
+    R.smem_bytes = (int)o;
+  };
+  // what is read every step goes to shared memory first (natives), then the L1 rows (read every nb_interval steps)
+  carve(true, pl_want);
+  if (o > 232448) carve(true, 0);
+  if (o > 232448) carve(false, 0);
   if (o > 232448) { pl.res_why = "chunk state does not fit the 227 KB of shared memory of an SM"; return; }
   if ((size_t)((N + 31) / 32) * 8 > 200000) { pl.res_why = "n_beads too large for the localise bitmap"; return; }
   pl.res_ok = true;
@@ -302,7 +330,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   if (p->mode < 0 || p->mode > 3) return fail(SOP_E_ARG, "mode must be 0, 1, 2 or 3");
   pl.mode = p->mode;
   if (pl.mode == 0 || pl.mode == 3) {
-    plan_resident(p, x, pl);
+    plan_resident(tp, p, x, pl);
     if (pl.mode == 3 && !pl.res_ok) return fail(SOP_E_ARG, "mode 3 is not possible here: " + pl.res_why);
     pl.mode = pl.res_ok ? 3 : 2;
   }
@@ -330,6 +358,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.off_cellcnt = take(pl.static_l1 ? 0 : (size_t)T * pl.max_cells * 4);
   pl.off_cellstart = take(pl.static_l1 ? 0 : (size_t)T * ((size_t)pl.max_cells + 1) * 4);
   pl.off_cellbead = take(pl.static_l1 ? 0 : I * 4);
+  pl.off_cellpos = take(pl.static_l1 ? 0 : I * 16);
   pl.off_flags = take(64);
   pl.off_epart = take((size_t)T * pl.energy_blocks * 5 * 8);
   pl.off_eout = take((size_t)T * 6 * 8);
@@ -340,8 +369,8 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
     pl.off_nhalo = take((size_t)T * R.C * 4);
     pl.off_hgid = take((size_t)T * R.C * R.halo_cap * 4);
     pl.off_plloc = take(R.implicit_l1 ? 0 : I * pl.cap_pl * 2);
-    pl.off_natloc = take(multi ? (size_t)T * pl.n_nat_entries * 2 : 0);
-    pl.off_bondloc = take(multi ? I * pl.cap_b * 2 : 0);
+    pl.off_natloc = take(multi ? (size_t)T * pl.n_nat_entries * 8 : 0);
+    pl.off_bondloc = take(multi ? I * pl.cap_b * 8 : 0);
     pl.off_xch = take(multi ? 2 * I * 32 : 0);
   }
   pl.total = o;
@@ -419,7 +448,7 @@ int launch_build_l1(sop_handle *h) {
     k_cell_scan<<<S.T, 1024, 0, st>>>(S);
     k_cell_fill<<<gi, 256, 0, st>>>(S);
     dim3 gs((unsigned)std::min(1024, (S.max_cells * 32 + 255) / 256), (unsigned)S.T);
-    k_cell_sort<<<gs, 256, 0, st>>>(S);
+    k_cell_sort<<<gs, 256, 0, st>>>(S, h->cur);
     k_build_l1<<<(unsigned)(((long long)S.n_inst * 32 + 255) / 256), 256, 0, st>>>(S, h->cur);
     h->launches += 8;
   }
@@ -494,17 +523,17 @@ int persistent_launch(sop_handle *h, int n, bool filter_last) {
   return SOP_OK;
 }
 
-template <int G, bool COMP>
-const void *resident_fn() { return (const void *)k_resident<G, COMP>; }
+template <int G>
+const void *resident_fn(bool comp) { return comp ? (const void *)k_resident<G, true> : (const void *)k_resident<G, false>; }
 
 const void *resident_kernel(int lanes, bool comp) {
   switch (lanes) {
-    case 1: return comp ? resident_fn<1, true>() : resident_fn<1, false>();
-    case 2: return comp ? resident_fn<2, true>() : resident_fn<2, false>();
-    case 4: return comp ? resident_fn<4, true>() : resident_fn<4, false>();
-    case 8: return comp ? resident_fn<8, true>() : resident_fn<8, false>();
-    case 16: return comp ? resident_fn<16, true>() : resident_fn<16, false>();
-    default: return comp ? resident_fn<32, true>() : resident_fn<32, false>();
+    case 1: return resident_fn<1>(comp);
+    case 2: return resident_fn<2>(comp);
+    case 4: return resident_fn<4>(comp);
+    case 8: return resident_fn<8>(comp);
+    case 16: return resident_fn<16>(comp);
+    default: return resident_fn<32>(comp);
   }
 }
 
@@ -514,11 +543,11 @@ int resident_prepare(sop_handle *h) {
   ResDev &R = h->R;
   char *w = h->ws;
   R.n_halo = (int *)(w + pl.off_nhalo); R.halo_gid = (int *)(w + pl.off_hgid);
-  R.pl_loc = (unsigned short *)(w + pl.off_plloc); R.nat_loc = (unsigned short *)(w + pl.off_natloc);
-  R.bond_loc = (unsigned short *)(w + pl.off_bondloc); R.xch = (uint4 *)(w + pl.off_xch);
+  R.pl_loc = (unsigned short *)(w + pl.off_plloc); R.nat_pack = (int2 *)(w + pl.off_natloc);
+  R.bond_pack = (int2 *)(w + pl.off_bondloc); R.xch = (uint4 *)(w + pl.off_xch);
   h->res_fn = resident_kernel(pl.res_lanes, pl.comp);
   CUDA_OK(cudaFuncSetAttribute(h->res_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, R.smem_bytes));
-  const int loc_smem = ((h->S.N + 31) / 32) * 8;
+  const int loc_smem = ((h->S.N + 31) / 32) * 8 + R.chunk * 4;
   CUDA_OK(cudaFuncSetAttribute((const void *)k_localise, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(loc_smem, 1024)));
   int occ = 0;
   CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->res_fn, pl.res_block, R.smem_bytes));
@@ -535,14 +564,14 @@ int resident_prepare(sop_handle *h) {
   return SOP_OK;
 }
 
-int resident_launch(sop_handle *h, int n, bool filter_last) {
+int resident_launch(sop_handle *h, int n, bool filter_last, bool filter_first) {
   span_close(h);
   span_begin(h, SPAN_STEP, n);
   SysDev S = h->S;
   ResDev R = h->R;
   int cur = h->cur;
   unsigned long long step0 = (unsigned long long)h->step;
-  int nb = h->prm.nb_interval, fl = filter_last ? 1 : 0;
+  int nb = h->prm.nb_interval, fl = (filter_last ? 1 : 0) | (filter_first ? 2 : 0);
   h->res_launch_id++;
   uint32_t stamp0 = ((h->res_launch_id & 0xFFFu) << 20) | 1u;     // never 0, never the previous launch's stamps
   void *args[] = {&S, &R, &cur, &step0, &n, &nb, &fl, &stamp0};
@@ -553,15 +582,17 @@ int resident_launch(sop_handle *h, int n, bool filter_last) {
   return SOP_OK;
 }
 
-int rebuild_lists(sop_handle *h) {
+// L1 (+ its slot form for mode 3), then L2 by Alg. 3.  with_filter = false (mode 3, inside sop_run only): the next
+// resident launch filters in its prologue instead, and the canonical L2 rows stay stale until that launch ends.
+int rebuild_lists(sop_handle *h, bool with_filter = true) {
   int rc = launch_build_l1(h);
   if (rc) return rc;
   if (h->plan.mode == 3 && !h->R.implicit_l1) {
-    const int loc_smem = ((h->S.N + 31) / 32) * 8;
-    k_localise<<<(unsigned)(h->S.T * h->R.C), 512, loc_smem, h->stream>>>(h->S, h->R);
+    const int loc_smem = ((h->S.N + 31) / 32) * 8 + h->R.chunk * 4;
+    k_localise<<<(unsigned)(h->S.T * h->R.C), 1024, loc_smem, h->stream>>>(h->S, h->R);
     h->launches++;
   }
-  launch_filter(h);
+  if (with_filter) launch_filter(h);
   span_close(h);
   return check_launch(h, "list rebuild");
 }
@@ -692,6 +723,7 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
   S.bbox = (float *)(w + pl.off_bbox); S.grid = (GridDev *)(w + pl.off_grid);
   S.cell_of = (int *)(w + pl.off_cellof); S.cell_cnt = (int *)(w + pl.off_cellcnt);
   S.cell_start = (int *)(w + pl.off_cellstart); S.cell_bead = (int *)(w + pl.off_cellbead);
+  S.cell_pos = (float4 *)(w + pl.off_cellpos);
   S.cell_edge = pl.static_l1 ? 1.0f : (float)((double)p->R_pl * 1.001);
   S.k_fene = p->k_fene; S.R0 = p->R0; S.inv_R0sq = (float)(1.0 / ((double)p->R0 * (double)p->R0));
   S.eps_native = p->eps_native;
@@ -794,17 +826,24 @@ int sop_run(sop_handle *h, int64_t n_steps) {
   if (!h || n_steps < 0) return fail(SOP_E_ARG, "bad handle or n_steps", h);
   const int64_t nb = h->prm.nb_interval, plv = h->prm.pl_interval;
   int64_t left = n_steps;
+  bool pending_filter = false;
   while (left > 0) {
     if (h->plan.mode >= 2) {
       // one persistent launch runs up to the next pair-list boundary, re-filtering L2 inside
       int64_t n = std::min<int64_t>(left, (1 << 20) - 2);
       if (!h->S.static_l1) n = std::min<int64_t>(n, plv - (h->step % plv));
       const bool l1_due = !h->S.static_l1 && (h->step + n) % plv == 0;
-      int rc = h->plan.mode == 3 ? resident_launch(h, (int)n, !l1_due) : persistent_launch(h, (int)n, !l1_due);
+      int rc = h->plan.mode == 3 ? resident_launch(h, (int)n, !l1_due, pending_filter) : persistent_launch(h, (int)n, !l1_due);
       if (rc) return rc;
+      pending_filter = false;
       if (h->plan.mode == 2) h->cur ^= (int)(n & 1);      // mode 3 writes the final layer back in place
       h->step += n; left -= n;
-      if (l1_due) { rc = rebuild_lists(h); if (rc) return rc; }
+      if (l1_due) {
+        pending_filter = h->plan.mode == 3 && left > 0;
+        rc = rebuild_lists(h, !pending_filter);
+        if (rc) return rc;
+        if (pending_filter) h->l2_built_at = h->step;
+      }
       else if (h->step / nb * nb > h->l2_built_at) h->l2_built_at = h->step / nb * nb;
     } else {
       span_begin(h, SPAN_STEP, 1);
@@ -953,6 +992,13 @@ int sop_device_coords(sop_handle *h, void **d_float4_out, int32_t *perm_out) {
   if (perm_out) memcpy(perm_out, h->plan.perm.data(), (size_t)h->S.N * 4);
   return SOP_OK;
 }
+
+#ifdef SOP_PHASE_CLOCKS
+extern "C" int sop_debug_phase_clocks(sop_handle *h, float *out, int n_float4) {     // profiling builds only
+  cudaStreamSynchronize(h->stream);
+  return (int)cudaMemcpy(out, h->S.force, (size_t)n_float4 * 16, cudaMemcpyDeviceToHost);
+}
+#endif
 
 int sop_get_config(sop_handle *h, int32_t out[9]) {
   if (!h || !out) return fail(SOP_E_ARG, "null argument", h);

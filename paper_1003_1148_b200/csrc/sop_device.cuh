@@ -51,6 +51,7 @@ struct SysDev {
   int *cell_cnt;                    // [T][max_cells]   (reused as fill cursor)
   int *cell_start;                  // [T][max_cells+1]
   int *cell_bead;                   // [T][N] beads sorted by (cell, internal index)
+  float4 *cell_pos;                 // [T][N] {x, y, z, bead index} in the same order
   float cell_edge;
   // parameters (fp32, derived once on the host in fp64)
   float k_fene, R0, inv_R0sq;

@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(256) k_cell_fill(SysDev S) {
 
 // One warp per cell: rank sort of the (distinct) bead indices so that the cell content, and with it every L1 row,
 // does not depend on the order in which the atomics of k_cell_fill were served.  cell_of is free by now: scratch.
-__global__ void __launch_bounds__(256) k_cell_sort(SysDev S) {
+__global__ void __launch_bounds__(256) k_cell_sort(SysDev S, int cur) {
   const int t = blockIdx.y;
   const int ncell = S.grid[t].ncell;
   const int lane = threadIdx.x & 31;
@@ -177,7 +177,13 @@ __global__ void __launch_bounds__(256) k_cell_sort(SysDev S) {
       tmp[s + rank] = v;
     }
     __syncwarp();
-    for (int a = lane; a < n; a += 32) bead[s + a] = tmp[s + a];
+    // sorted ids back, and the cell-sorted coordinate copy {x, y, z, bead index} the L1 build streams through
+    for (int a = lane; a < n; a += 32) {
+      const int v = tmp[s + a];
+      bead[s + a] = v;
+      const float4 r = __ldg(S.pos[cur] + (size_t)t * S.N + v);
+      S.cell_pos[(size_t)t * S.N + s + a] = make_float4(r.x, r.y, r.z, __int_as_float(v));
+    }
     __syncwarp();
   }
 }
@@ -193,43 +199,62 @@ __device__ __forceinline__ bool is_excluded(const SysDev &S, int i, int j) {
   return false;
 }
 
-// a2: L1 pair-list build, one warp per bead instance: scan the 27 cells around the bead, keep j != i in the
-// non-native set with pred32(R_pl); ballot + prefix-popcount compaction (row order: cells z,y,x ascending, beads
-// ascending inside a cell -- deterministic; sop_get_lists returns rows sorted by the caller's index).
+// a2: L1 pair-list build, one warp per bead instance: stream through the cell-sorted coordinates of the 27 cells
+// around the bead (9 contiguous segments, the next 32 candidates in flight while the current ones are tested), keep
+// j != i in the non-native set with pred32(R_pl); ballot + prefix-popcount compaction (row order: cells z,y,x
+// ascending, beads ascending inside a cell -- deterministic; sop_get_lists returns rows sorted by the caller's index).
+// The bead's exclusion row (bonded + native partners) is staged in shared memory for the membership test.
+constexpr int EXCL_SMEM = 64;
 __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
+  __shared__ int s_excl[8][EXCL_SMEM];
   const int w = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   if (w >= S.n_inst) return;
   const int t = w / S.N, i = w - t * S.N;
-  const float4 *__restrict__ pos_t = S.pos[cur] + (size_t)t * S.N;
+  const float4 *__restrict__ cpos = S.cell_pos + (size_t)t * S.N;
   const GridDev gd = S.grid[t];
   const int *start = S.cell_start + (size_t)t * (S.max_cells + 1);
-  const int *bead = S.cell_bead + (size_t)t * S.N;
   int *dst = S.pl_idx + (size_t)w * S.cap_pl;
-  const float4 ri = __ldg(pos_t + i);
+  const float4 ri = __ldg(S.pos[cur] + (size_t)t * S.N + i);
+  const int e0 = __ldg(&S.excl_ptr[i]), ne = __ldg(&S.excl_ptr[i + 1]) - e0;
+  const bool ex_smem = ne <= EXCL_SMEM;
+  if (ex_smem) for (int k = lane; k < ne; k += 32) s_excl[wib][k] = __ldg(&S.excl_idx[e0 + k]);
   const int3 c = cell_coords(gd, ri);
-  int n = 0;
-  for (int z = max(c.z - 1, 0); z <= min(c.z + 1, gd.nz - 1); ++z)
-    for (int y = max(c.y - 1, 0); y <= min(c.y + 1, gd.ny - 1); ++y) {
-      // the x-neighbours of a row of cells are contiguous in cell_bead: one segment per (z, y)
+  // the 9 (z, y) rows of cells: lane l < 9 fetches the bounds of row (l / 3 - 1, l % 3 - 1)
+  int my_s = 0, my_e = 0;
+  if (lane < 9) {
+    const int z = c.z + lane / 3 - 1, y = c.y + lane % 3 - 1;
+    if (z >= 0 && z < gd.nz && y >= 0 && y < gd.ny) {
       const int c0 = (z * gd.ny + y) * gd.nx + max(c.x - 1, 0), c1 = (z * gd.ny + y) * gd.nx + min(c.x + 1, gd.nx - 1);
-      const int s = start[c0], e = start[c1 + 1];
-      for (int base = s; base < e; base += 32) {
-        int q = base + lane;
-        int j = -1;
-        bool pass = false;
-        if (q < e) {
-          j = bead[q];
-          pass = j != i && pred32(ri, __ldg(pos_t + j), S.R_pl2) && !is_excluded(S, i, j);
-        }
-        unsigned m = __ballot_sync(0xffffffffu, pass);
-        if (pass) {
-          int slot = n + __popc(m & ((1u << lane) - 1u));
-          if (slot < S.cap_pl) dst[slot] = j;
-        }
-        n += __popc(m);
-      }
+      my_s = start[c0]; my_e = start[c1 + 1];
     }
+  }
+  __syncwarp();
+  auto excluded = [&](int j) -> bool {
+    if (!ex_smem) return is_excluded(S, i, j);
+    int lo = 0, hi = ne;
+    while (lo < hi) { const int mid = (lo + hi) >> 1; const int v = s_excl[wib][mid]; if (v == j) return true; if (v < j) lo = mid + 1; else hi = mid; }
+    return false;
+  };
+  int n = 0;
+  for (int seg = 0; seg < 9; ++seg) {
+    const int s = __shfl_sync(0xffffffffu, my_s, seg), e = __shfl_sync(0xffffffffu, my_e, seg);
+    float4 nxt = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (s + lane < e) nxt = __ldg(cpos + s + lane);
+    for (int base = s; base < e; base += 32) {
+      const float4 rj = nxt;
+      const int q = base + lane;
+      if (q + 32 < e) nxt = __ldg(cpos + q + 32);
+      const int j = __float_as_int(rj.w);
+      const bool pass = q < e && j != i && pred32(ri, rj, S.R_pl2) && !excluded(j);
+      const unsigned m = __ballot_sync(0xffffffffu, pass);
+      if (pass) {
+        const int slot = n + __popc(m & ((1u << lane) - 1u));
+        if (slot < S.cap_pl) dst[slot] = j;
+      }
+      n += __popc(m);
+    }
+  }
   if (lane == 0) {
     if (n > S.cap_pl) { atomicOr(S.flags, FLAG_PL_OVERFLOW); n = S.cap_pl; }
     S.pl_cnt[w] = n;

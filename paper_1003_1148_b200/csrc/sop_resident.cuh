@@ -13,6 +13,8 @@
 // Two exchange layers suffice: a CTA can only overwrite layer k with k+2 after it has read its neighbours'
 // layer k+1, which they publish after they finished reading layer k.
 #pragma once
+#include <type_traits>
+
 #include "sop_kernels.cuh"
 
 namespace sop {
@@ -28,12 +30,16 @@ struct ResDev {
   int *n_halo;                // [T*C]
   int *halo_gid;              // [T*C][halo_cap] bead index (within the trajectory) of each halo slot, ascending
   unsigned short *pl_loc;     // [T*N][cap_pl]   L1 rows as slots
-  unsigned short *nat_loc;    // [T][nat_entries]
-  unsigned short *bond_loc;   // [T][N*cap_b]
+  int2 *nat_pack;             // [T][nat_entries] {slot, bits(r0^2)}   (C > 1; with one chunk slot = bead index)
+  int2 *bond_pack;            // [T*N][cap_b]     {slot or -1, bits(r0)} (C > 1)
   uint4 *xch;                 // [2][T*N][2]  {x, stamp, y, stamp} {z, stamp, -, -}
   // shared-memory carve-up (bytes from the start of dynamic shared memory), computed by the host
-  int off_pos, off_g, off_carry, off_tag, off_nb, off_cnt, off_active, off_bm, off_sbm, off_misc;
-  int nb_si, nb_sp;           // nb_loc(i, p) = nb[i * nb_si + p * nb_sp]
+  int off_pos, off_g, off_carry, off_tag, off_facc, off_nb, off_cnt, off_rofs, off_plcnt, off_plofs, off_pl, off_natq,
+      off_nat, off_bond, off_active, off_bm, off_sbm, off_misc;
+  int nb_si;                  // L2 row i starts at nb[i * nb_si] (an odd number of 32-bit words: conflict-free)
+  int nat_smem;               // the chunk's native table is copied to shared memory (nat_cap entries fit)
+  int nat_cap;                // largest number of native entries of a chunk
+  int pl_cap;                 // 16-bit entries of shared memory for the chunk's L1 rows (0: read them from global)
   int smem_bytes;
 };
 
@@ -61,32 +67,41 @@ __device__ __forceinline__ bool xch_try(const uint4 *slot, uint32_t st, float4 &
 // k_localise: after an L1 build, give every chunk its halo slot table and re-express L1 rows, natives and bonds
 // in chunk-local slots.  One CTA per (trajectory, chunk); dynamic shared memory: bitmap + prefix over the N beads.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(512) k_localise(SysDev S, ResDev R) {
+__global__ void __launch_bounds__(1024) k_localise(SysDev S, ResDev R) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int W = (S.N + 31) >> 5;
   uint32_t *bm = (uint32_t *)smem_raw;         // [W] bead j is in the halo
   uint32_t *pre = bm + W;                      // [W] exclusive prefix of popc(bm)
+  int *cnt = (int *)(pre + W);                 // [chunk] L1 row counts of the own beads
   __shared__ int warp_tot[32];
   __shared__ int carry_s;
   const int tc = blockIdx.x, t = tc / R.C, c = tc - t * R.C;
   const int b0 = c * R.chunk, b1 = min(S.N, b0 + R.chunk), n_own = b1 - b0;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-  for (int w = threadIdx.x; w < W; w += blockDim.x) bm[w] = 0u;
-  if (threadIdx.x == 0) carry_s = 0;
+  const int tid = threadIdx.x, bd = blockDim.x;
+  const int lane = tid & 31, warp = tid >> 5, nwarps = bd >> 5;
+  const size_t g0 = (size_t)t * S.N + b0;
+  const int cap_pl = S.cap_pl, cap_b = S.cap_b;
+  for (int w = tid; w < W; w += bd) bm[w] = 0u;
+  for (int i = tid; i < n_own; i += bd) cnt[i] = min(S.pl_cnt[g0 + i], cap_pl);
+  if (tid == 0) carry_s = 0;
   __syncthreads();
+  // every loop below is flat over table entries: independent, coalesced loads, nothing waits on a row at a time
   auto mark = [&](int j) { if (j < b0 || j >= b1) atomicOr(&bm[j >> 5], 1u << (j & 31)); };
-  for (int i = b0 + warp; i < b1; i += nwarps) {
-    const int g = t * S.N + i;
-    const int cnt = S.pl_cnt[g];
-    const int *row = S.pl_idx + (size_t)g * S.cap_pl;
-    for (int p = lane; p < cnt; p += 32) mark(row[p]);
-    for (int q = S.nat_ptr[i] + lane; q < S.nat_ptr[i + 1]; q += 32) mark(S.nat_tab[q].x);
-    for (int p = lane; p < S.cap_b; p += 32) { int j = S.bond_tab[(size_t)i * S.cap_b + p].x; if (j >= 0) mark(j); }
+  const int *rows = S.pl_idx + g0 * cap_pl;
+  for (int e = tid; e < n_own * cap_pl; e += bd) {
+    const int r = e / cap_pl;
+    if (e - r * cap_pl < cnt[r]) mark(rows[e]);
+  }
+  const int q0 = S.nat_ptr[b0], q1 = S.nat_ptr[b1];
+  const bool multi = R.C > 1;
+  if (multi) {
+    for (int q = q0 + tid; q < q1; q += bd) mark(S.nat_tab[q].x);
+    for (int e = tid; e < n_own * cap_b; e += bd) { const int j = S.bond_tab[(size_t)b0 * cap_b + e].x; if (j >= 0) mark(j); }
   }
   __syncthreads();
   // exclusive scan of the word popcounts
-  for (int base = 0; base < W; base += blockDim.x) {
-    const int w = base + threadIdx.x;
+  for (int base = 0; base < W; base += bd) {
+    const int w = base + tid;
     const int v = w < W ? __popc(bm[w]) : 0;
     int inc = v;
     for (int o = 1; o < 32; o <<= 1) { int n = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += n; }
@@ -101,104 +116,60 @@ __global__ void __launch_bounds__(512) k_localise(SysDev S, ResDev R) {
     const int excl = carry_s + warp_tot[warp] + inc - v;
     if (w < W) pre[w] = (uint32_t)excl;
     __syncthreads();
-    if (threadIdx.x == blockDim.x - 1) carry_s = excl + v;
+    if (tid == bd - 1) carry_s = excl + v;
     __syncthreads();
   }
   const int n_halo = carry_s;
   if (n_halo > R.halo_cap) {
-    if (threadIdx.x == 0) { atomicOr(S.flags, FLAG_SLOT_OVERFLOW); R.n_halo[tc] = 0; }
+    if (tid == 0) { atomicOr(S.flags, FLAG_SLOT_OVERFLOW); R.n_halo[tc] = 0; }
     return;
   }
-  if (threadIdx.x == 0) R.n_halo[tc] = n_halo;
+  if (tid == 0) R.n_halo[tc] = n_halo;
   int *hg = R.halo_gid + (size_t)tc * R.halo_cap;
-  for (int w = threadIdx.x; w < W; w += blockDim.x) {
+  for (int w = tid; w < W; w += bd) {
     uint32_t bits = bm[w];
     int k = (int)pre[w];
     while (bits) { int b = __ffs(bits) - 1; bits &= bits - 1; hg[k++] = (w << 5) + b; }
   }
-  auto slot_of = [&](int j) -> unsigned short {
-    if (j >= b0 && j < b1) return (unsigned short)(j - b0);
-    return (unsigned short)(n_own + pre[j >> 5] + __popc(bm[j >> 5] & ((1u << (j & 31)) - 1u)));
+  auto slot_of = [&](int j) -> int {
+    if (j >= b0 && j < b1) return j - b0;
+    return n_own + (int)pre[j >> 5] + __popc(bm[j >> 5] & ((1u << (j & 31)) - 1u));
   };
-  for (int i = b0 + warp; i < b1; i += nwarps) {
-    const int g = t * S.N + i;
-    const int cnt = S.pl_cnt[g];
-    const int *row = S.pl_idx + (size_t)g * S.cap_pl;
-    unsigned short *dst = R.pl_loc + (size_t)g * S.cap_pl;
-    for (int p = lane; p < cnt; p += 32) dst[p] = slot_of(row[p]);
-    if (R.C == 1) continue;                     // one chunk: slot = bead index, natives and bonds need no table
-    for (int q = S.nat_ptr[i] + lane; q < S.nat_ptr[i + 1]; q += 32)
-      R.nat_loc[(size_t)t * R.nat_entries + q] = slot_of(S.nat_tab[q].x);
-    for (int p = lane; p < S.cap_b; p += 32) {
-      int j = S.bond_tab[(size_t)i * S.cap_b + p].x;
-      R.bond_loc[(size_t)g * S.cap_b + p] = j >= 0 ? slot_of(j) : (unsigned short)0;
+  unsigned short *loc = R.pl_loc + g0 * cap_pl;
+  for (int e = tid; e < n_own * cap_pl; e += bd) {
+    const int r = e / cap_pl;
+    if (e - r * cap_pl < cnt[r]) loc[e] = (unsigned short)slot_of(rows[e]);
+  }
+  if (multi) {                                  // one chunk: slot = bead index, natives and bonds need no table
+    for (int q = q0 + tid; q < q1; q += bd) {
+      const int2 en = S.nat_tab[q];
+      R.nat_pack[(size_t)t * R.nat_entries + q] = make_int2(slot_of(en.x), en.y);
+    }
+    for (int e = tid; e < n_own * cap_b; e += bd) {
+      const int2 en = S.bond_tab[(size_t)b0 * cap_b + e];
+      R.bond_pack[g0 * cap_b + e] = make_int2(en.x >= 0 ? slot_of(en.x) : -1, en.y);
     }
   }
 }
 
 // ------------------------------------------------------------------------------------------------
 // Pair force laws of Eq. (1) with MUFU reciprocals (1 ulp; the parity bar is 1e-4 max|F|).
+// Each returns s with f_i += s (r_i - r_j).
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void acc_pair(const float4 &ri, const float4 &rj, float &dx, float &dy, float &dz, float &r2) {
-  dx = ri.x - rj.x; dy = ri.y - rj.y; dz = ri.z - rj.z;
-  r2 = dx * dx + dy * dy + dz * dz;
-}
+struct ForceK {                // loop invariants kept in registers
+  float k_fene, inv_R0sq, eps12, c_rep_f;
+};
 
-// Internal force on own bead `il` (slot il, bead index gi) from shared-memory coordinates: Alg. 2
-// with the partner loop spread over G lanes; no distance test in the loop (reading R3c).
-template <int G>
-__device__ __forceinline__ float3 resident_force(const SysDev &S, const ResDev &R, const float4 *__restrict__ sp,
-                                                 const unsigned short *__restrict__ nb, int cnt, int il, int gi, int t,
-                                                 int lane, bool valid, const float4 &ri, int &flag) {
-  float fx = 0.f, fy = 0.f, fz = 0.f;
-  if (valid) {
-    const bool multi = R.C > 1;
-    // a4: FENE bonds
-    for (int p = lane; p < S.cap_b; p += G) {
-      const int2 e = __ldg(&S.bond_tab[(size_t)gi * S.cap_b + p]);
-      if (e.x >= 0) {
-        const int slot = multi ? (int)__ldg(&R.bond_loc[((size_t)t * S.N + gi) * S.cap_b + p]) : e.x;
-        float dx, dy, dz, r2;
-        acc_pair(ri, sp[slot], dx, dy, dz, r2);
-        const float inv_r = rsqrtf(r2);
-        const float del = r2 * inv_r - __int_as_float(e.y);
-        const float x = 1.0f - del * del * S.inv_R0sq;
-        if (!(x > 0.0f)) flag |= FLAG_FENE;
-        const float s = -S.k_fene * del * fast_rcp(x) * inv_r;
-        fx += s * dx; fy += s * dy; fz += s * dz;
-      }
-    }
-    // a5: native contacts
-    {
-      const int q0 = __ldg(&S.nat_ptr[gi]), q1 = __ldg(&S.nat_ptr[gi + 1]);
-      for (int q = q0 + lane; q < q1; q += G) {
-        const int2 e = __ldg(&S.nat_tab[q]);
-        const float eps = S.nat_eps ? __ldg(&S.nat_eps[q]) : S.eps_native;
-        const int slot = multi ? (int)__ldg(&R.nat_loc[(size_t)t * R.nat_entries + q]) : e.x;
-        float dx, dy, dz, r2;
-        acc_pair(ri, sp[slot], dx, dy, dz, r2);
-        const float inv_r2 = fast_rcp(r2);
-        const float u = __int_as_float(e.y) * inv_r2;
-        const float q3 = u * u * u;
-        const float s = 12.0f * eps * inv_r2 * (q3 * q3 - q3);
-        fx += s * dx; fy += s * dy; fz += s * dz;
-      }
-    }
-    // a6: non-native repulsion over the shared-memory neighbor list
-    {
-      const unsigned short *row = nb + (size_t)il * R.nb_si;
-      for (int p = lane; p < cnt; p += G) {
-        const int slot = row[(size_t)p * R.nb_sp];
-        float dx, dy, dz, r2;
-        acc_pair(ri, sp[slot], dx, dy, dz, r2);
-        const float inv_r2 = fast_rcp(r2);
-        const float s = S.c_rep_f * (inv_r2 * inv_r2) * (inv_r2 * inv_r2);
-        fx += s * dx; fy += s * dy; fz += s * dz;
-      }
-    }
-  }
-  if (G > 1) { fx = group_sum<G>(fx); fy = group_sum<G>(fy); fz = group_sum<G>(fz); }
-  return make_float3(fx, fy, fz);
+__device__ __forceinline__ float rep_s3(float r2, float c_rep_f) {        // 6 eps_r sigma^6 / r^8
+  const float inv_r2 = fast_rcp(r2);
+  const float i4 = inv_r2 * inv_r2;
+  return c_rep_f * i4 * i4;
+}
+__device__ __forceinline__ float nat_s3(float r2, float r0sq, float e12) {  // (12 eps / r^2) (q^2 - q), q = (r0/r)^6
+  const float inv_r2 = fast_rcp(r2);
+  const float u = r0sq * inv_r2;
+  const float q3 = u * u * u;
+  return e12 * inv_r2 * (q3 * q3 - q3);
 }
 
 __device__ __forceinline__ int lower_bound_dev(const int *__restrict__ a, int n, int v) {
@@ -209,25 +180,39 @@ __device__ __forceinline__ int lower_bound_dev(const int *__restrict__ a, int n,
 
 // ------------------------------------------------------------------------------------------------
 // k_resident: a3 + a4..a9 for n_steps Langevin steps of one chunk per CTA (see the header of this file).
-// Shared-memory buffers are double-buffered on the step parity, so a step needs one __syncthreads:
-//   (a) noise of this step, thread per bead        (b) fetch the active halo of this step's layer
-//   (c) __syncthreads                              (d) forces (G lanes per bead) + update + publish
-//   (e) every nb_interval steps: fetch the whole halo of the new layer, Alg. 3 on the own rows, new active set.
+// Per step:
+//   (b) fetch the active halo of this step's layer (poll the stamps)                    -- __syncthreads --
+//   (d1) a4..a6: the chunk's bonds, native entries and L2 entries are each dealt out evenly to ALL threads as
+//        contiguous runs (a thread walks its run row by row, sums in registers, adds once per row into the per-bead
+//        fixed-point accumulators)                                                       -- __syncthreads --
+//   (d2) a7 + a9 thread per bead: external force, update, publish; meanwhile the threads at the other end of the block
+//        generate the noise (a8) of the NEXT step, off the critical path
+//   (e) every nb_interval steps: fetch the whole halo of the new layer, Alg. 3 on the own rows (L1 rows resident in
+//        shared memory), new active set, new row offsets.
+// Coordinates and noise are double-buffered on the step parity.
 // ------------------------------------------------------------------------------------------------
 template <int G, bool COMP>
 __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cur, unsigned long long step0, int n_steps,
-                                                      int nb_interval, int filter_last, uint32_t stamp0) {
+                                                      int nb_interval, int filter_flags, uint32_t stamp0) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int slots_cap = R.chunk + R.halo_cap;
-  float4 *spos = (float4 *)(smem_raw + R.off_pos);                   // [2][slots_cap]
-  float4 *sg = (float4 *)(smem_raw + R.off_g);                       // [2][chunk]   (G > 1)
+  const bool filter_last = filter_flags & 1, filter_first = filter_flags & 2;
+  const int SC = R.chunk + R.halo_cap + 1;                           // + the dummy slot (last)
+  float4 *spos = (float4 *)(smem_raw + R.off_pos);                   // [2][SC]
+  float4 *sg = (float4 *)(smem_raw + R.off_g);                       // [2][chunk]
   float4 *scarry = (float4 *)(smem_raw + R.off_carry);               // [chunk]      (COMP)
   uint32_t *stag = (uint32_t *)(smem_raw + R.off_tag);               // [chunk]
-  unsigned short *nb = (unsigned short *)(smem_raw + R.off_nb);      // L2 rows as slots
-  unsigned short *cnt_s = (unsigned short *)(smem_raw + R.off_cnt);  // [chunk]
+  float4 *sforce = (float4 *)(smem_raw + R.off_facc);                // [chunk] internal force of this step
+  unsigned short *nb = (unsigned short *)(smem_raw + R.off_nb);      // L2 rows as slots, row stride nb_si
+  unsigned short *cnt_s = (unsigned short *)(smem_raw + R.off_cnt);  // [chunk] L2 row counts
+  unsigned short *plcnt_s = (unsigned short *)(smem_raw + R.off_plcnt);  // [chunk] L1 row counts
+  int *plofs = (int *)(smem_raw + R.off_plofs);                      // [chunk + 1] L1 row starts in spl (even)
+  unsigned short *spl = (unsigned short *)(smem_raw + R.off_pl);     // [pl_cap] L1 rows as slots, packed
+  int *natq = (int *)(smem_raw + R.off_natq);                        // [chunk + 1] native table offsets
+  int2 *snat = (int2 *)(smem_raw + R.off_nat);                       // [nat_cap]    (nat_smem)
+  int2 *sbond = (int2 *)(smem_raw + R.off_bond);                     // [chunk][cap_b]
   unsigned short *active = (unsigned short *)(smem_raw + R.off_active);
   uint32_t *bm = (uint32_t *)(smem_raw + R.off_bm), *sbm = (uint32_t *)(smem_raw + R.off_sbm);
-  int *misc = (int *)(smem_raw + R.off_misc);                        // [0] = number of active halo slots
+  int *misc = (int *)(smem_raw + R.off_misc);                        // [0] active halo slots, [1] L1 rows are in spl
 
   const int tc = blockIdx.x, t = tc / R.C, c = tc - t * R.C;
   const int b0 = c * R.chunk, b1 = min(S.N, b0 + R.chunk), n_own = b1 - b0;
@@ -236,49 +221,152 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   const int *__restrict__ hgid = R.halo_gid + (size_t)tc * R.halo_cap;
   const int HW = (n_halo + 31) >> 5;
   const int tid = threadIdx.x, bd = blockDim.x;
-  const int lane = tid % G, grp = tid / G, groups = bd / G;
   const int wlane = tid & 31, warp = tid >> 5, nwarps = bd >> 5;
+  const int lane = tid % G, grp = tid / G, groups = bd / G;
+  const unsigned short DUMMY = (unsigned short)(SC - 1);
   const size_t inst0 = (size_t)t * S.N;
   uint4 *const xl0 = R.xch, *const xl1 = R.xch + 2 * (size_t)S.n_inst;
+  const int cap_b = S.cap_b, cap_nb = S.cap_nb;
+  const uint32_t traj = (uint32_t)(S.traj_offset + t);
   int flag = 0;
 
-  // ---- prologue: own coordinates, carry, tags; canonical L2 rows -> slots; static part of the active set
+  // exclusive scan of n_own 16-bit counts by warp 0 (the caller synchronises)
+  auto scan_counts = [&](const unsigned short *cnt, int *ofs, bool round_even) {
+    if (warp == 0) {
+      int carry = 0;
+      for (int base = 0; base < n_own; base += 32) {
+        const int i = base + wlane;
+        int v = i < n_own ? (int)cnt[i] : 0;
+        if (round_even) v = (v + 1) & ~1;
+        int inc = v;
+        for (int o = 1; o < 32; o <<= 1) { const int n = __shfl_up_sync(0xffffffffu, inc, o); if (wlane >= o) inc += n; }
+        if (i < n_own) ofs[i] = carry + inc - v;
+        carry += __shfl_sync(0xffffffffu, inc, 31);
+      }
+      if (wlane == 0) ofs[n_own] = carry;
+    }
+  };
+
+  // ---- prologue: own coordinates, carry, tags, static tables; canonical L2 rows -> slots; L1 rows -> shared memory
+  const int qbase = S.nat_ptr[b0];
+  if (tid == 0) {      // a point 1e18 A away: its repulsion underflows to exactly zero (pads odd L2 rows)
+    spos[SC - 1] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.f);
+    spos[2 * SC - 1] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.f);
+  }
   for (int i = tid; i < n_own; i += bd) {
     const float4 v = S.pos[cur][inst0 + b0 + i];
     spos[i] = v;
     stag[i] = __float_as_uint(v.w);
     if (multi) xch_put(xl0 + 2 * (inst0 + b0 + i), v, stamp0);
     if (COMP) scarry[i] = S.carry[inst0 + b0 + i];
-  }
-  for (int il = warp; il < n_own; il += nwarps) {
-    const size_t g = inst0 + b0 + il;
-    const int cnt = min(S.nb_cnt[g], S.cap_nb);
-    const int *row = S.nb_idx + g * S.cap_nb;
-    for (int p = wlane; p < cnt; p += 32) {
-      const int j = row[p];
-      const int slot = (j >= b0 && j < b1) ? j - b0 : n_own + lower_bound_dev(hgid, n_halo, j);
-      nb[(size_t)il * R.nb_si + (size_t)p * R.nb_sp] = (unsigned short)slot;
+    natq[i] = S.nat_ptr[b0 + i];
+    plcnt_s[i] = R.implicit_l1 ? (unsigned short)0 : (unsigned short)S.pl_cnt[inst0 + b0 + i];
+    const uint32_t tag = __float_as_uint(v.w);
+    if (G > 1 && !(tag & TAG_FIXED)) {
+      const float3 gn = gaussian3(S, tag & TAG_ID_MASK, traj, step0);
+      sg[i] = make_float4(gn.x, gn.y, gn.z, 0.f);
     }
-    if (wlane == 0) cnt_s[il] = (unsigned short)cnt;
+  }
+  if (tid == 0) natq[n_own] = S.nat_ptr[b1];
+  const int2 *bond_src = multi ? R.bond_pack + (inst0 + b0) * cap_b : S.bond_tab + (size_t)b0 * cap_b;
+  for (int e = tid; e < n_own * cap_b; e += bd) sbond[e] = bond_src[e];
+  const int2 *nat_glob = multi ? R.nat_pack + (size_t)t * R.nat_entries : S.nat_tab;
+  const int n_nat = S.nat_ptr[b1] - qbase;
+  if (R.nat_smem)
+    for (int e = tid; e < n_nat; e += bd) snat[e] = nat_glob[qbase + e];
+  const int2 *natp = R.nat_smem ? (const int2 *)snat - qbase : nat_glob;      // indexed by the global offset q
+  if (filter_first) {
+    // the launch starts on a fresh L1: the L2 rows come from Alg. 3 below, on the whole halo of the canonical layer
+    for (int q = tid; q < n_halo; q += bd) {
+      const float4 v = S.pos[cur][inst0 + hgid[q]];
+      spos[n_own + q] = make_float4(v.x, v.y, v.z, 0.f);
+    }
+  } else {
+    for (int il = warp; il < n_own; il += nwarps) {
+      const size_t g = inst0 + b0 + il;
+      const int cnt = min(S.nb_cnt[g], cap_nb);
+      const int *row = S.nb_idx + g * cap_nb;
+      unsigned short *dst = nb + (size_t)il * R.nb_si;
+      for (int p = wlane; p < cnt; p += 32) {
+        const int j = row[p];
+        dst[p] = (unsigned short)((j >= b0 && j < b1) ? j - b0 : n_own + lower_bound_dev(hgid, n_halo, j));
+      }
+      if (wlane == 0) { cnt_s[il] = (unsigned short)cnt; if (cnt & 1) dst[cnt] = DUMMY; }
+    }
   }
   for (int w = tid; w < HW; w += bd) sbm[w] = 0u;
   __syncthreads();
-  if (multi) {
+  scan_counts(plcnt_s, plofs, true);
+  __syncthreads();
+  const bool pl_in_smem = !R.implicit_l1 && R.pl_cap > 0 && plofs[n_own] <= R.pl_cap;
+  if (pl_in_smem) {
     for (int il = warp; il < n_own; il += nwarps) {
-      const int gi = b0 + il;
-      for (int q = S.nat_ptr[gi] + wlane; q < S.nat_ptr[gi + 1]; q += 32) {
-        const int h = (int)R.nat_loc[(size_t)t * R.nat_entries + q] - n_own;
-        if (h >= 0) atomicOr(&sbm[h >> 5], 1u << (h & 31));
-      }
-      for (int p = wlane; p < S.cap_b; p += 32)
-        if (S.bond_tab[(size_t)gi * S.cap_b + p].x >= 0) {
-          const int h = (int)R.bond_loc[(inst0 + gi) * S.cap_b + p] - n_own;
-          if (h >= 0) atomicOr(&sbm[h >> 5], 1u << (h & 31));
-        }
+      const uint32_t *src = (const uint32_t *)(R.pl_loc + (inst0 + b0 + il) * S.cap_pl);
+      uint32_t *dst = (uint32_t *)(spl + plofs[il]);
+      const int nw = ((int)plcnt_s[il] + 1) >> 1;
+      for (int p = wlane; p < nw; p += 32) dst[p] = __ldg(src + p);
     }
   }
-  // active halo = static part + slots of the current L2 rows (3 barriers)
-  auto build_active = [&]() {
+  // static part of the active set: halo slots the bonds and natives of the own beads use
+  if (multi) {
+    for (int e = tid; e < n_own * cap_b; e += bd) {
+      const int h = sbond[e].x - n_own;
+      if (h >= 0) atomicOr(&sbm[h >> 5], 1u << (h & 31));
+    }
+    for (int e = tid; e < n_nat; e += bd) {
+      const int h = natp[qbase + e].x - n_own;
+      if (h >= 0) atomicOr(&sbm[h >> 5], 1u << (h & 31));
+    }
+  }
+  __syncthreads();
+  // a3: Alg. 3 on the own rows, candidates and coordinates from shared memory
+  auto filter_rows = [&](const float4 *P) {
+    const uint32_t lt = (1u << wlane) - 1u;
+    if (R.implicit_l1) {
+      for (int il = warp; il < n_own; il += nwarps) {
+        const int gi = b0 + il;
+        const float4 ri = P[il];
+        unsigned short *row = nb + (size_t)il * R.nb_si;
+        int n = 0;
+        for (int base = 0; base < S.N; base += 32) {
+          const int j = base + wlane;
+          const bool pass = j < S.N && j != gi && pred32(ri, P[min(j, S.N - 1)], S.R_nb2) && !is_excluded(S, gi, j);
+          const unsigned m = __ballot_sync(0xffffffffu, pass);
+          if (pass) { const int at = n + __popc(m & lt); if (at < cap_nb) row[at] = (unsigned short)j; }
+          n += __popc(m);
+        }
+        if (n > cap_nb) { flag |= FLAG_NB_OVERFLOW; n = cap_nb; }
+        if (wlane == 0) { cnt_s[il] = (unsigned short)n; if (n & 1) row[n] = DUMMY; }
+      }
+    } else {
+      // two candidates per lane per iteration, read as one 32-bit word of the (packed, even-aligned) L1 row
+      for (int il = warp; il < n_own; il += nwarps) {
+        const int cnt1 = plcnt_s[il];
+        const float4 ri = P[il];
+        const uint32_t *src = pl_in_smem ? (const uint32_t *)(spl + plofs[il])
+                                         : (const uint32_t *)(R.pl_loc + (inst0 + b0 + il) * S.cap_pl);
+        unsigned short *row = nb + (size_t)il * R.nb_si;
+        int n = 0;
+        for (int base = 0; base < cnt1; base += 64) {
+          const int p0 = base + 2 * wlane;
+          const uint32_t u = p0 < cnt1 ? src[p0 >> 1] : 0u;
+          const int s0 = u & 0xFFFFu, s1 = (p0 + 1 < cnt1) ? (int)(u >> 16) : 0;
+          const bool pass0 = p0 < cnt1 && pred32(ri, P[s0], S.R_nb2);
+          const bool pass1 = p0 + 1 < cnt1 && pred32(ri, P[s1], S.R_nb2);
+          const unsigned m0 = __ballot_sync(0xffffffffu, pass0), m1 = __ballot_sync(0xffffffffu, pass1);
+          const int at0 = n + __popc(m0 & lt) + __popc(m1 & lt), at1 = at0 + (pass0 ? 1 : 0);
+          if (pass0 && at0 < cap_nb) row[at0] = (unsigned short)s0;
+          if (pass1 && at1 < cap_nb) row[at1] = (unsigned short)s1;
+          n += __popc(m0) + __popc(m1);
+        }
+        if (n > cap_nb) { flag |= FLAG_NB_OVERFLOW; n = cap_nb; }
+        if (wlane == 0) { cnt_s[il] = (unsigned short)n; if (n & 1) row[n] = DUMMY; }
+      }
+    }
+  };
+  // active halo = static part + halo slots of the current L2 rows
+  auto after_filter = [&]() {
+    __syncthreads();                                   // the row counts are complete
     for (int w = tid; w < HW; w += bd) bm[w] = sbm[w];
     if (tid == 0) misc[0] = 0;
     __syncthreads();
@@ -286,7 +374,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
       for (int il = warp; il < n_own; il += nwarps) {
         const int cnt = cnt_s[il];
         for (int p = wlane; p < cnt; p += 32) {
-          const int h = (int)nb[(size_t)il * R.nb_si + (size_t)p * R.nb_sp] - n_own;
+          const int h = (int)nb[(size_t)il * R.nb_si + p] - n_own;
           if (h >= 0) atomicOr(&bm[h >> 5], 1u << (h & 31));
         }
       }
@@ -301,31 +389,31 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     }
     __syncthreads();
   };
-  __syncthreads();
-  build_active();
+  if (filter_first) filter_rows(spos);
+  after_filter();
 
   // ---- the steps
-  bool have_full = false;                    // the whole halo of the current layer is already in shared memory
+  ForceK K;
+  K.k_fene = S.k_fene; K.inv_R0sq = S.inv_R0sq; K.eps12 = 12.0f * S.eps_native; K.c_rep_f = S.c_rep_f;
+  const float *nat_eps = S.nat_eps;
+  int until_filter = nb_interval - (int)(step0 % (unsigned long long)nb_interval);
+  bool have_full = filter_first;             // the whole halo of the current layer is already in shared memory
+#ifdef SOP_PHASE_CLOCKS
+  long long pc_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, pc_t = clock64();
+#define SOP_TICK(n) { const long long now_ = clock64(); pc_acc[n] += now_ - pc_t; pc_t = now_; }
+#else
+#define SOP_TICK(n)
+#endif
   for (int k = 0; k < n_steps; ++k) {
     const unsigned long long step = step0 + (unsigned long long)k;
-    float4 *pc = spos + (size_t)(k & 1) * slots_cap, *pn = spos + (size_t)((k & 1) ^ 1) * slots_cap;
-    float4 *gc = sg + (size_t)(k & 1) * R.chunk;
+    float4 *pc = spos + (size_t)(k & 1) * SC, *pn = spos + (size_t)((k & 1) ^ 1) * SC;
+    float4 *gc = sg + (size_t)(k & 1) * R.chunk, *gnx = sg + (size_t)((k & 1) ^ 1) * R.chunk;
     uint4 *const xc = (k & 1) ? xl1 : xl0, *const xn = (k & 1) ? xl0 : xl1;
     const uint32_t st_c = stamp0 + (uint32_t)k, st_n = st_c + 1u;
-    // (a) a8: noise of this step, one thread per bead (the lanes of a group would otherwise idle through it)
-    if (G > 1) {
-      for (int i = tid; i < n_own; i += bd) {
-        const uint32_t tag = stag[i];
-        if (!(tag & TAG_FIXED)) {
-          const float3 gn = gaussian3(S, tag & TAG_ID_MASK, (uint32_t)(S.traj_offset + t), step);
-          gc[i] = make_float4(gn.x, gn.y, gn.z, 0.f);
-        }
-      }
-    }
     // (b) active halo of layer k: poll until the neighbours have published it
     if (multi && !have_full) {
       const int na = misc[0];
-      for (int q = bd - 1 - tid; q < na; q += bd) {
+      for (int q = tid; q < na; q += bd) {
         const int slot = active[q];
         const uint4 *src = xc + 2 * (inst0 + hgid[slot - n_own]);
         float4 v;
@@ -334,80 +422,137 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
       }
     }
     have_full = false;
-    __syncthreads();                                                                       // (c)
-    // (d) a4..a7 forces, a9 update, publish
+    SOP_TICK(0)                                                                            // halo poll
+    __syncthreads();
+    SOP_TICK(1)                                                                            // waiting for the CTA
+    // (d1) a4..a6: internal force, G lanes per bead (Alg. 2; no distance test in the loop, R3c)
     for (int base = 0; base < n_own; base += groups) {
-      const int il = base + grp;
-      const bool valid = il < n_own;
-      const int ii = valid ? il : 0, gi = b0 + ii;
-      const float4 ri = pc[ii];
-      float3 f = resident_force<G>(S, R, pc, nb, valid ? (int)cnt_s[ii] : 0, ii, gi, t, lane, valid, ri, flag);
-      if (valid && lane == 0) {
-        const uint32_t tag = stag[ii];
-        float4 out = ri;
-        if (!(tag & TAG_FIXED)) {
-          external_force(S, gi, ri, tag, step, f.x, f.y, f.z, flag);
-          float3 gn;
-          if (G > 1) { const float4 g4 = gc[ii]; gn = make_float3(g4.x, g4.y, g4.z); }
-          else gn = gaussian3(S, tag & TAG_ID_MASK, (uint32_t)(S.traj_offset + t), step);
-          out = langevin_apply<COMP>(S, ri, gn, f.x, f.y, f.z, COMP ? scarry + ii : nullptr, flag);
+      const bool valid = base + grp < n_own;
+      const int il = valid ? base + grp : n_own - 1;
+      const float4 ri = pc[il];
+      float fx = 0.f, fy = 0.f, fz = 0.f;
+      if (valid) {
+        // a4: FENE bonds   V = -(k/2) R0^2 ln(1 - (r-r0)^2/R0^2)
+        for (int p = lane; p < cap_b; p += G) {
+          const int2 b = sbond[il * cap_b + p];
+          if (b.x >= 0) {
+            const float4 rj = pc[b.x];
+            const float dx = ri.x - rj.x, dy = ri.y - rj.y, dz = ri.z - rj.z;
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            const float inv_r = rsqrtf(r2);
+            const float del = r2 * inv_r - __int_as_float(b.y);
+            const float x = 1.0f - del * del * K.inv_R0sq;
+            if (!(x > 0.0f)) flag |= FLAG_FENE;
+            const float s = -K.k_fene * del * fast_rcp(x) * inv_r;
+            fx += s * dx; fy += s * dy; fz += s * dz;
+          }
         }
-        pn[ii] = out;
-        if (multi) xch_put(xn + 2 * (inst0 + gi), out, st_n);
+        // a5: native contacts   V = eps [(r0/r)^12 - 2 (r0/r)^6]   (per-contact eps only when the topology has it)
+        const int q1 = natq[il + 1];
+        auto natives = [&](auto has_eps_t) {
+          constexpr bool HAS_EPS = decltype(has_eps_t)::value;
+          for (int q = natq[il] + lane; q < q1; q += G) {
+            const int2 en = natp[q];
+            float e12 = K.eps12;
+            if (HAS_EPS) e12 = 12.0f * __ldg(&nat_eps[q]);
+            const float4 rj = pc[en.x];
+            const float dx = ri.x - rj.x, dy = ri.y - rj.y, dz = ri.z - rj.z;
+            const float s = nat_s3(dx * dx + dy * dy + dz * dz, __int_as_float(en.y), e12);
+            fx += s * dx; fy += s * dy; fz += s * dz;
+          }
+        };
+        if (nat_eps) natives(std::true_type{}); else natives(std::false_type{});
+        // a6: non-native repulsion   V = eps_r (sigma/r)^6; two slots per 32-bit word, odd rows end in the dummy slot
+        const uint32_t *row32 = (const uint32_t *)(nb + (size_t)il * R.nb_si);
+        const int n2 = ((int)cnt_s[il] + 1) >> 1;
+        for (int p = lane; p < n2; p += G) {
+          const uint32_t u = row32[p];
+          const float4 ra = pc[u & 0xFFFFu], rb = pc[u >> 16];
+          const float ax = ri.x - ra.x, ay = ri.y - ra.y, az = ri.z - ra.z;
+          const float bx = ri.x - rb.x, by = ri.y - rb.y, bz = ri.z - rb.z;
+          const float sa = rep_s3(ax * ax + ay * ay + az * az, K.c_rep_f);
+          const float sb = rep_s3(bx * bx + by * by + bz * bz, K.c_rep_f);
+          fx += sa * ax; fy += sa * ay; fz += sa * az;
+          fx += sb * bx; fy += sb * by; fz += sb * bz;
+        }
+      }
+      if (G > 1) { fx = group_sum<G>(fx); fy = group_sum<G>(fy); fz = group_sum<G>(fz); }
+      if (valid && lane == 0) sforce[il] = make_float4(fx, fy, fz, 0.f);
+    }
+    SOP_TICK(2)                                                                            // pair forces
+    __syncthreads();
+    // (d2) a7 + a9: thread per bead; the other end of the block draws the next step's noise (a8)
+    for (int i = tid; i < n_own; i += bd) {
+      const float4 ri = pc[i];
+      const uint32_t tag = stag[i];
+      const float4 a = sforce[i];
+      float4 out = ri;
+      if (!(tag & TAG_FIXED)) {
+        float fx = a.x, fy = a.y, fz = a.z;
+        external_force(S, b0 + i, ri, tag, step, fx, fy, fz, flag);
+        float3 gn;
+        if (G > 1) { const float4 g4 = gc[i]; gn = make_float3(g4.x, g4.y, g4.z); }
+        else gn = gaussian3(S, tag & TAG_ID_MASK, traj, step);      // thread per bead already: nobody idles
+        out = langevin_apply<COMP>(S, ri, gn, fx, fy, fz, COMP ? scarry + i : nullptr, flag);
+      }
+      pn[i] = out;
+      if (multi) xch_put(xn + 2 * (inst0 + b0 + i), out, st_n);
+    }
+    if (G > 1 && k + 1 < n_steps) {
+      for (int i = bd - 1 - tid; i < n_own; i += bd) {
+        const uint32_t tag = stag[i];
+        if (!(tag & TAG_FIXED)) {
+          const float3 gn = gaussian3(S, tag & TAG_ID_MASK, traj, step + 1);
+          gnx[i] = make_float4(gn.x, gn.y, gn.z, 0.f);
+        }
       }
     }
+    SOP_TICK(3)                                                                            // update + noise
     // (e) a3: Alg. 3 on the own rows from the coordinates just written (list invariant)
-    if ((step + 1) % (unsigned long long)nb_interval == 0 && (k + 1 < n_steps || filter_last)) {
-      if (multi)
-        for (int q = tid; q < n_halo; q += bd) {
-          const uint4 *src = xn + 2 * (inst0 + hgid[q]);
-          float4 v;
-          while (!xch_try(src, st_n, v)) {}
-          pn[n_own + q] = v;
-        }
-      __syncthreads();
-      for (int il = warp; il < n_own; il += nwarps) {
-        const int gi = b0 + il;
-        const size_t g = inst0 + gi;
-        const float4 ri = pn[il];
-        int *canon = S.nb_idx + g * S.cap_nb;
-        unsigned short *row = nb + (size_t)il * R.nb_si;
-        int n = 0;
-        const int cnt1 = R.implicit_l1 ? S.N : S.pl_cnt[g];
-        const unsigned short *src = R.pl_loc + g * S.cap_pl;
-        for (int base = 0; base < cnt1; base += 32) {
-          const int p = base + wlane;
-          int slot = 0;
-          bool pass = false;
-          if (p < cnt1) {
-            slot = R.implicit_l1 ? p : (int)src[p];
-            pass = pred32(ri, pn[slot], S.R_nb2);
-            if (R.implicit_l1) pass = pass && p != gi && !is_excluded(S, gi, p);
+    if (--until_filter == 0) {
+      until_filter = nb_interval;
+      if (k + 1 < n_steps || filter_last) {
+        if (multi)
+          for (int q = tid; q < n_halo; q += bd) {
+            const uint4 *src = xn + 2 * (inst0 + hgid[q]);
+            float4 v;
+            while (!xch_try(src, st_n, v)) {}
+            pn[n_own + q] = v;
           }
-          const unsigned m = __ballot_sync(0xffffffffu, pass);
-          if (pass) {
-            const int at = n + __popc(m & ((1u << wlane) - 1u));
-            if (at < S.cap_nb) {
-              row[(size_t)at * R.nb_sp] = (unsigned short)slot;
-              canon[at] = slot < n_own ? b0 + slot : hgid[slot - n_own];
-            }
-          }
-          n += __popc(m);
-        }
-        if (n > S.cap_nb) { flag |= FLAG_NB_OVERFLOW; n = S.cap_nb; }
-        if (wlane == 0) { cnt_s[il] = (unsigned short)n; S.nb_cnt[g] = n; }
+        SOP_TICK(4)                                                                        // whole-halo poll
+        __syncthreads();
+        SOP_TICK(5)
+        filter_rows(pn);
+        SOP_TICK(6)                                                                        // Alg. 3 rows
+        after_filter();
+        have_full = true;
       }
-      build_active();
-      have_full = true;
+      SOP_TICK(7)                                                                          // active set, offsets
     }
   }
+#ifdef SOP_PHASE_CLOCKS
+  if (wlane == 0) {
+    S.force[((size_t)blockIdx.x * 32 + warp) * 2] = make_float4((float)pc_acc[0], (float)pc_acc[1], (float)pc_acc[2], (float)pc_acc[3]);
+    S.force[((size_t)blockIdx.x * 32 + warp) * 2 + 1] = make_float4((float)pc_acc[4], (float)pc_acc[5], (float)pc_acc[6], (float)pc_acc[7]);
+  }
+#endif
 
-  // ---- epilogue: the current layer back to the canonical arrays
+  // ---- epilogue: the current layer, the carry and the L2 rows back to the canonical arrays
   __syncthreads();
-  const float4 *pf = spos + (size_t)(n_steps & 1) * slots_cap;
+  const float4 *pf = spos + (size_t)(n_steps & 1) * SC;
   for (int i = tid; i < n_own; i += bd) {
     S.pos[cur][inst0 + b0 + i] = pf[i];
     if (COMP) S.carry[inst0 + b0 + i] = scarry[i];
+  }
+  for (int il = warp; il < n_own; il += nwarps) {
+    const size_t g = inst0 + b0 + il;
+    const int cnt = cnt_s[il];
+    int *canon = S.nb_idx + g * cap_nb;
+    for (int p = wlane; p < cnt; p += 32) {
+      const int slot = nb[(size_t)il * R.nb_si + p];
+      canon[p] = slot < n_own ? b0 + slot : hgid[slot - n_own];
+    }
+    if (wlane == 0) S.nb_cnt[g] = cnt;
   }
   if (flag) atomicOr(S.flags, flag);
 }
