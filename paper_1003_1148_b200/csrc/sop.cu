@@ -320,7 +320,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   int lanes = p->lanes_per_bead;
   if (lanes == 0) {
     lanes = 32;
-    while (lanes > 1 && inst * lanes > 1200000LL) lanes >>= 1;   // ~4 resident threads' worth of the chip
+    while (lanes > 1 && inst * lanes > 600000LL) lanes >>= 1;    // measured on cfg 4: fewer lanes once the chip is full
   }
   if (lanes != 1 && lanes != 2 && lanes != 4 && lanes != 8 && lanes != 16 && lanes != 32)
     return fail(SOP_E_ARG, "lanes_per_bead must be 0 or a power of two <= 32");
@@ -332,9 +332,10 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   if (pl.mode == 0 || pl.mode == 3) {
     plan_resident(tp, p, x, pl);
     if (pl.mode == 3 && !pl.res_ok) return fail(SOP_E_ARG, "mode 3 is not possible here: " + pl.res_why);
-    pl.mode = pl.res_ok ? 3 : 2;
+    // fallback: the streaming kernels; one launch per step once the chip is full (measured on cfg 4), else persistent
+    pl.mode = pl.res_ok ? 3 : (inst > 100000 ? 1 : 2);
   }
-  pl.energy_blocks = (int)std::min<long long>(64, ((long long)N * 8 + 255) / 256);
+  pl.energy_blocks = (int)std::min<long long>(296, ((long long)N * 8 + 255) / 256);
 
   // workspace
   size_t o = 0;

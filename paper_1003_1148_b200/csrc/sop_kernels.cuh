@@ -239,20 +239,27 @@ __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
   int n = 0;
   for (int seg = 0; seg < 9; ++seg) {
     const int s = __shfl_sync(0xffffffffu, my_s, seg), e = __shfl_sync(0xffffffffu, my_e, seg);
-    float4 nxt = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (s + lane < e) nxt = __ldg(cpos + s + lane);
-    for (int base = s; base < e; base += 32) {
-      const float4 rj = nxt;
-      const int q = base + lane;
-      if (q + 32 < e) nxt = __ldg(cpos + q + 32);
-      const int j = __float_as_int(rj.w);
-      const bool pass = q < e && j != i && pred32(ri, rj, S.R_pl2) && !excluded(j);
-      const unsigned m = __ballot_sync(0xffffffffu, pass);
-      if (pass) {
-        const int slot = n + __popc(m & ((1u << lane) - 1u));
-        if (slot < S.cap_pl) dst[slot] = j;
+    // 128 candidates per iteration: four independent 16-byte loads per lane in flight, then four ordered compactions
+    for (int base = s; base < e; base += 128) {
+      float4 rj[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int q = base + 32 * u + lane;
+        rj[u] = q < e ? __ldg(cpos + q) : make_float4(0.f, 0.f, 0.f, __int_as_float(i));
       }
-      n += __popc(m);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (base + 32 * u >= e) break;
+        const int q = base + 32 * u + lane;
+        const int j = __float_as_int(rj[u].w);
+        const bool pass = q < e && j != i && pred32(ri, rj[u], S.R_pl2) && !excluded(j);
+        const unsigned m = __ballot_sync(0xffffffffu, pass);
+        if (pass) {
+          const int slot = n + __popc(m & ((1u << lane) - 1u));
+          if (slot < S.cap_pl) dst[slot] = j;
+        }
+        n += __popc(m);
+      }
     }
   }
   if (lane == 0) {

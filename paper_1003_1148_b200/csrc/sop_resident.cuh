@@ -86,11 +86,21 @@ __global__ void __launch_bounds__(1024) k_localise(SysDev S, ResDev R) {
   if (tid == 0) carry_s = 0;
   __syncthreads();
   // every loop below is flat over table entries: independent, coalesced loads, nothing waits on a row at a time
-  auto mark = [&](int j) { if (j < b0 || j >= b1) atomicOr(&bm[j >> 5], 1u << (j & 31)); };
+  // test before the atomic: neighbours share most of their halo, so nearly every bit is already set
+  auto mark = [&](int j) {
+    if (j < b0 || j >= b1) { const uint32_t bit = 1u << (j & 31); if (!(((volatile uint32_t *)bm)[j >> 5] & bit)) atomicOr(&bm[j >> 5], bit); }
+  };
   const int *rows = S.pl_idx + g0 * cap_pl;
-  for (int e = tid; e < n_own * cap_pl; e += bd) {
-    const int r = e / cap_pl;
-    if (e - r * cap_pl < cnt[r]) mark(rows[e]);
+  const int n_rows_e = n_own * cap_pl;
+  for (int e0 = tid; e0 < n_rows_e; e0 += 4 * bd) {          // four independent loads in flight per thread
+    int v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int e = e0 + u * bd, r = e / cap_pl;
+      v[u] = (e < n_rows_e && e - r * cap_pl < cnt[r]) ? rows[e] : -1;
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (v[u] >= 0) mark(v[u]);
   }
   const int q0 = S.nat_ptr[b0], q1 = S.nat_ptr[b1];
   const bool multi = R.C > 1;
@@ -136,9 +146,15 @@ __global__ void __launch_bounds__(1024) k_localise(SysDev S, ResDev R) {
     return n_own + (int)pre[j >> 5] + __popc(bm[j >> 5] & ((1u << (j & 31)) - 1u));
   };
   unsigned short *loc = R.pl_loc + g0 * cap_pl;
-  for (int e = tid; e < n_own * cap_pl; e += bd) {
-    const int r = e / cap_pl;
-    if (e - r * cap_pl < cnt[r]) loc[e] = (unsigned short)slot_of(rows[e]);
+  for (int e0 = tid; e0 < n_rows_e; e0 += 4 * bd) {
+    int v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int e = e0 + u * bd, r = e / cap_pl;
+      v[u] = (e < n_rows_e && e - r * cap_pl < cnt[r]) ? rows[e] : -1;
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (v[u] >= 0) loc[e0 + u * bd] = (unsigned short)slot_of(v[u]);
   }
   if (multi) {                                  // one chunk: slot = bead index, natives and bonds need no table
     for (int q = q0 + tid; q < q1; q += bd) {
