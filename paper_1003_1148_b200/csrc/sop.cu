@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <string>
@@ -191,7 +192,7 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
     keys.erase(std::unique(keys.begin(), keys.end()), keys.end());
     for (uint64_t k : keys) cnt[(int)(k >> 32)]++;
     const int worst = *std::max_element(cnt.begin(), cnt.end());
-    halo_cap = ((int)(worst * 1.25) + 64 + 31) / 32 * 32;
+    halo_cap = ((int)(worst * 1.15) + 32 + 31) / 32 * 32;
   }
   R.halo_cap = halo_cap;
   const long long slots = (long long)chunk + halo_cap;
@@ -232,12 +233,23 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
     R.off_misc = take(64);
     R.smem_bytes = (int)o;
   };
+  // implicit L1: the same region holds the in-kernel cell grid (2 x (cells + 1) ints + 2 x chunk shorts)
+  if (pl.static_l1) pl_want = (2 * (RES_GRID_CELLS + 1) * 4 + 4 * chunk + 64) / 2;
   // what is read every step goes to shared memory first (natives), then the L1 rows (read every nb_interval steps)
   carve(true, pl_want);
-  if (o > 232448) carve(true, 0);
-  if (o > 232448) carve(false, 0);
+  if (o > 232448 && pl.static_l1) carve(false, pl_want);
+  if (o > 232448 && !pl.static_l1) {
+    // the L1 rows get what is left (the kernel reads them from global memory if a chunk's rows do not fit at run time)
+    carve(true, 0);
+    const long long left = (232448 - (long long)o) / 2 - 16;
+    if (left > 4 * chunk) carve(true, (int)std::min<long long>(pl_want, left));
+  }
+  if (o > 232448 && !pl.static_l1) carve(false, 0);
   if (o > 232448) { pl.res_why = "chunk state does not fit the 227 KB of shared memory of an SM"; return; }
   if ((size_t)((N + 31) / 32) * 8 > 200000) { pl.res_why = "n_beads too large for the localise bitmap"; return; }
+  if (getenv("SOP_DEBUG_PLAN"))
+    fprintf(stderr, "[sop plan] mode 3: C=%d chunk=%d lanes=%d block=%d halo_cap=%d cap_nb=%d cap_pl=%d nat_smem=%d pl_cap=%d smem=%d B\n",
+            R.C, R.chunk, pl.res_lanes, pl.res_block, R.halo_cap, pl.cap_nb, pl.cap_pl, R.nat_smem, R.pl_cap, R.smem_bytes);
   pl.res_ok = true;
 }
 

@@ -341,3 +341,64 @@ def test_full_config3_shell_indented(mode):
 @pytest.mark.parametrize("mode", [0, 1])
 def test_full_config4_lattice(mode):
     full_check(4, mode=mode)
+
+
+# ---------------------------------------------------------------------------------------------- more mode-3 coverage
+@pytest.mark.parametrize("var", [dict(mode=1, lanes_per_bead=4), dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=45)],
+                         ids=str)
+def test_per_contact_native_eps(var):
+    """topology.native_eps (one eps per native contact, PAPER.md:241 eps_n) on every kernel path."""
+    w = gen.tiny(150, 21, R_pl=20.0)
+    eps = (0.5 + np.random.default_rng(5).random(len(w.native))).astype(np.float32)
+    s = sop().Sop(w.xyz, w.bonds, w.native, w.params, native_eps=eps, **var)
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, w.params, native_eps=eps)
+    check_forces(s, o, w.xyz[None])
+    check_energies(s.get_energies(), o.get_energies())
+    s.run(100); o.run(100)
+    assert np.abs(s.get_coords() - o.get_coords()).max() <= 1e-3
+
+
+def test_mode3_long_run_across_pair_list_rebuilds():
+    """350 steps = 3 pair-list rebuilds inside one sop_run (the in-kernel first filter after each) against three
+    separate runs that end on the rebuild boundaries (k_filter path) and against the oracle's lists at the end."""
+    w = gen.two_chains(150, 3, R_pl=20.0)
+    a = sop().from_workload(w, mode=3, chunk_beads=60); a.run(350)
+    b = sop().from_workload(w, mode=3, chunk_beads=60); b.run(100); b.run(200); b.run(50)
+    assert np.array_equal(a.get_coords(), b.get_coords())
+    o = sopo.from_workload(w)
+    xa = a.get_coords()
+    assert a.get_lists(1)[2] == 300 and a.get_lists(2)[2] == 350
+    # L2 was filtered at step 350 from the L1 of step 300: compare with the oracle driven to the same state
+    o.run(350)
+    assert np.abs(xa - o.get_coords()).max() <= 5e-3          # 350 steps: fp32 vs fp64 drift, still far below a bond length
+    e_gpu = a.get_energies()
+    assert np.isfinite(e_gpu).all()
+
+
+def test_mode3_halo_overflow_is_an_error_not_a_truncation():
+    """Compress the structure after create: more beads enter a chunk's 20 A halo than its slot table holds."""
+    m = sop()
+    w = gen.tiny(400, 12, R_pl=20.0)
+    s = m.from_workload(w, mode=3, chunk_beads=50)
+    x = (w.xyz[None] * np.float32(0.55)).astype(np.float32)     # 6x the density: every list and halo grows
+    with pytest.raises(m.SopError) as ei:
+        s.set_coords(x)
+        s.run(10)
+        s.sync()
+    assert ei.value.code in (-3, -4)                            # list / halo overflow (or a crushed bond caught first)
+
+
+def test_ensemble_means_energy_and_rg_within_3_standard_errors():
+    """north_star: long-run ensemble means (energy, radius of gyration) of GPU and oracle agree within 3 SE.
+    64 independent trajectories of a small globule, 2000 steps, same Philox streams on both sides (the test does
+    not rely on the trajectories staying close, only on the ensemble)."""
+    w = gen.tiny(64, 31)
+    T, n = 64, 2000
+    s = sop().from_workload(w, n_traj=T, mode=3); s.run(n)
+    o = sopo.from_workload(w, n_traj=T); o.run(n)
+    xg, xo = s.get_coords().astype(np.float64), o.get_coords()
+    rg = lambda x: np.sqrt(((x - x.mean(axis=1, keepdims=True)) ** 2).sum(axis=2).mean(axis=1))
+    eg, eo = s.get_energies()[:, 5], o.get_energies()[:, 5]
+    for a, b in ((rg(xg), rg(xo)), (eg, eo)):
+        se = math.sqrt(a.var(ddof=1) / T + b.var(ddof=1) / T)
+        assert abs(a.mean() - b.mean()) <= 3 * se, (a.mean(), b.mean(), se)
