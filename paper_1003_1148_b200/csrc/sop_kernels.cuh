@@ -89,7 +89,7 @@ __global__ void k_grid_setup(SysDev S) {
     long long tot = 1;
     for (int a = 0; a < 3; ++a) { n[a] = (int)floorf(ext[a] / edge) + 1; tot *= n[a]; }
     if (tot <= S.max_cells) break;
-    edge *= 1.25f;                       // cells may only grow: any edge >= cell_edge keeps the 27-cell scan complete
+    edge *= 1.25f;                       // cells may only grow: any edge >= cell_edge keeps the scan complete
   }
   GridDev gd;
   gd.ox = lo[0]; gd.oy = lo[1]; gd.oz = lo[2];
@@ -200,11 +200,13 @@ __device__ __forceinline__ bool is_excluded(const SysDev &S, int i, int j) {
 }
 
 // a2: L1 pair-list build, one warp per bead instance: stream through the cell-sorted coordinates of the 27 cells
-// around the bead (9 contiguous segments, the next 32 candidates in flight while the current ones are tested), keep
+// around the bead ((2 SPAN + 1)^2 contiguous segments, the next 32 candidates in flight while the current ones are tested), keep
 // j != i in the non-native set with pred32(R_pl); ballot + prefix-popcount compaction (row order: cells z,y,x
 // ascending, beads ascending inside a cell -- deterministic; sop_get_lists returns rows sorted by the caller's index).
 // The bead's exclusion row (bonded + native partners) is staged in shared memory for the membership test.
 constexpr int EXCL_SMEM = 64;
+constexpr int CELL_SPAN = 1;            // cell edge = R_pl / CELL_SPAN, scan (2 SPAN + 1)^3 cells.  SPAN = 2 tests 42 % fewer
+                                        // candidates but measured slower on cfg 3 (114 vs 89 us: 25 short segments, 8x the cells)
 __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
   __shared__ int s_excl[8][EXCL_SMEM];
   const int w = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
@@ -220,12 +222,13 @@ __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
   const bool ex_smem = ne <= EXCL_SMEM;
   if (ex_smem) for (int k = lane; k < ne; k += 32) s_excl[wib][k] = __ldg(&S.excl_idx[e0 + k]);
   const int3 c = cell_coords(gd, ri);
-  // the 9 (z, y) rows of cells: lane l < 9 fetches the bounds of row (l / 3 - 1, l % 3 - 1)
+  // the (z, y) rows of cells: lane l fetches the bounds of row (l / SIDE - SPAN, l % SIDE - SPAN)
   int my_s = 0, my_e = 0;
-  if (lane < 9) {
-    const int z = c.z + lane / 3 - 1, y = c.y + lane % 3 - 1;
+  constexpr int SIDE = 2 * CELL_SPAN + 1, NSEG = SIDE * SIDE;
+  if (lane < NSEG) {
+    const int z = c.z + lane / SIDE - CELL_SPAN, y = c.y + lane % SIDE - CELL_SPAN;
     if (z >= 0 && z < gd.nz && y >= 0 && y < gd.ny) {
-      const int c0 = (z * gd.ny + y) * gd.nx + max(c.x - 1, 0), c1 = (z * gd.ny + y) * gd.nx + min(c.x + 1, gd.nx - 1);
+      const int c0 = (z * gd.ny + y) * gd.nx + max(c.x - CELL_SPAN, 0), c1 = (z * gd.ny + y) * gd.nx + min(c.x + CELL_SPAN, gd.nx - 1);
       my_s = start[c0]; my_e = start[c1 + 1];
     }
   }
@@ -237,7 +240,7 @@ __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
     return false;
   };
   int n = 0;
-  for (int seg = 0; seg < 9; ++seg) {
+  for (int seg = 0; seg < NSEG; ++seg) {
     const int s = __shfl_sync(0xffffffffu, my_s, seg), e = __shfl_sync(0xffffffffu, my_e, seg);
     // 128 candidates per iteration: four independent 16-byte loads per lane in flight, then four ordered compactions
     for (int base = s; base < e; base += 128) {

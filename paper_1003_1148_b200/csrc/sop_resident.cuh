@@ -481,28 +481,53 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         if (n & 1) row[n] = DUMMY;
       }
     } else {
-      // two candidates per lane per iteration, read as one 32-bit word of the (packed, even-aligned) L1 row
-      for (int il = warp; il < n_own; il += nwarps) {
-        const int cnt1 = plcnt_s[il];
+      // LPR lanes per row (as many as the block has per own bead, a power of two): a lane tests a contiguous run of
+      // 64 candidates per round into a 64-bit mask -- no ballots, no popcounts per candidate -- then the lanes of the
+      // row exchange their counts and write their survivors in row order (Alg. 3 keeps the L1 order)
+      int LPR = 1;
+      while (LPR < 32 && 2 * LPR * n_own <= bd) LPR <<= 1;
+      const int frow = tid / LPR, flane = tid & (LPR - 1), fgroups = bd / LPR;
+      for (int base = 0; base < n_own; base += fgroups) {
+        const bool valid = base + frow < n_own;
+        const int il = valid ? base + frow : n_own - 1;
+        const int cnt1 = valid ? (int)plcnt_s[il] : 0;
+        const int nw = (cnt1 + 1) >> 1;
         const float4 ri = P[il];
         const uint32_t *src = pl_in_smem ? (const uint32_t *)(spl + plofs[il])
                                          : (const uint32_t *)(R.pl_loc + (inst0 + b0 + il) * S.cap_pl);
         unsigned short *row = nb + (size_t)il * R.nb_si;
+        const int rounds = __reduce_max_sync(0xffffffffu, (nw + 32 * LPR - 1) / (32 * LPR));
         int n = 0;
-        for (int base = 0; base < cnt1; base += 64) {
-          const int p0 = base + 2 * wlane;
-          const uint32_t u = p0 < cnt1 ? src[p0 >> 1] : 0u;
-          const int s0 = u & 0xFFFFu, s1 = (p0 + 1 < cnt1) ? (int)(u >> 16) : 0;
-          const bool pass0 = p0 < cnt1 && pred32(ri, P[s0], S.R_nb2);
-          const bool pass1 = p0 + 1 < cnt1 && pred32(ri, P[s1], S.R_nb2);
-          const unsigned m0 = __ballot_sync(0xffffffffu, pass0), m1 = __ballot_sync(0xffffffffu, pass1);
-          const int at0 = n + __popc(m0 & lt) + __popc(m1 & lt), at1 = at0 + (pass0 ? 1 : 0);
-          if (pass0 && at0 < cap_nb) row[at0] = (unsigned short)s0;
-          if (pass1 && at1 < cap_nb) row[at1] = (unsigned short)s1;
-          n += __popc(m0) + __popc(m1);
+        for (int r = 0; r < rounds; ++r) {
+          // the (up to 32 LPR) words of this round are split evenly: at most 32 words = 64 candidates per lane
+          const int rw0 = r * 32 * LPR, rwn = min(32 * LPR, nw - rw0), per = (max(rwn, 0) + LPR - 1) / LPR;
+          const int w0 = rw0 + flane * per;
+          unsigned long long mask = 0ull;
+          const int wend = min(per, rwn - flane * per);
+#pragma unroll 4
+          for (int k2 = 0; k2 < wend; ++k2) {
+            const uint32_t u = src[w0 + k2];
+            const bool pa = pred32(ri, P[u & 0xFFFFu], S.R_nb2);
+            const bool pb = 2 * (w0 + k2) + 1 < cnt1 && pred32(ri, P[u >> 16], S.R_nb2);
+            mask |= (unsigned long long)(pa ? 1u : 0u) << (2 * k2);
+            mask |= (unsigned long long)(pb ? 1u : 0u) << (2 * k2 + 1);
+          }
+          const int mine = __popcll(mask);
+          int incl = mine;
+          for (int o = 1; o < LPR; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o, LPR); if (flane >= o) incl += v; }
+          const int total = __shfl_sync(0xffffffffu, incl, LPR - 1, LPR);
+          int at = n + incl - mine;
+          while (mask) {
+            const int bit = __ffsll((long long)mask) - 1;
+            mask &= mask - 1;
+            const uint32_t u = src[w0 + (bit >> 1)];
+            if (at < cap_nb) row[at] = (unsigned short)((bit & 1) ? (u >> 16) : (u & 0xFFFFu));
+            ++at;
+          }
+          n += total;
         }
         if (n > cap_nb) { flag |= FLAG_NB_OVERFLOW; n = cap_nb; }
-        if (wlane == 0) { cnt_s[il] = (unsigned short)n; if (n & 1) row[n] = DUMMY; }
+        if (valid && flane == 0) { cnt_s[il] = (unsigned short)n; if (n & 1) row[n] = DUMMY; }
       }
     }
   };
