@@ -110,6 +110,12 @@ int sop_set_coords(sop_handle *, const float *xyz /*HOST [T][N][3]*/);   /* rebu
 /* Eq. (1) term by term + external terms, per trajectory: fene, native, rep (over the current
  * L2, each pair once), pull, tip, total.  fp32 pair terms, fp64 accumulation. */
 int sop_get_energies(sop_handle *, double *e_out /*HOST [T][6]*/);
+/* Observables of the paper's applications, per trajectory, reduced on the device (PAPER.md:261 force-extension curves
+ * f(R); :312-314 force-indentation): o[0] = radius of gyration, o[1] = end-to-end distance X between the first fixed
+ * bead (else bead 0) and the first pulled bead (else bead N-1), o[2] = cantilever force summed over the pulled beads
+ * kappa (v s - (r_p - a_p).n)  (= r_f t at zero displacement, r_f = kappa v), o[3] = force resisting the
+ * indenter sum_i F_i^tip . tip_dir.  fp32 terms, fp64 sums. */
+int sop_get_observables(sop_handle *, double *o_out /*HOST [T][4]*/);
 /* Deterministic force (no noise) at the current coordinates with the current L2, incl. external terms. */
 int sop_get_forces(sop_handle *, float *f_out /*HOST [T][N][3]*/);
 /* Row counts and rows (ascending caller index j, padded with -1 to cap) of trajectory traj.

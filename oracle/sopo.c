@@ -587,6 +587,57 @@ int sopo_get_energies(sopo_handle *h, double *e_out) {
   return status;
 }
 
+/* Observables the paper's applications plot (PAPER.md:261 force-extension curves f(R), Fig. 3; :312-314
+ * force-indentation), per trajectory, plain definitions:
+ *   o[0] = Rg   = sqrt( (1/N) sum_i |r_i - r_cm|^2 ),  r_cm = (1/N) sum_i r_i
+ *   o[1] = X    = |r_b - r_a|,  a = first fixed bead (else bead 0), b = first pulled bead (else bead N-1)
+ *   o[2] = f    = sum over pulled beads of kappa (v s - (r_p - a_p).n)      (cantilever force; = r_f t at zero
+ *                 displacement, r_f = kappa v)
+ *   o[3] = f_tip = sum_i F_i^tip . n_tip = dV_tip / d(advance)              (force resisting the indenter, reading R8) */
+int sopo_get_observables(sopo_handle *h, double *o_out) {
+  if (!h || !o_out) return SOPO_E_ARG;
+  const sopo_params *p = &h->p;
+  const int32_t N = h->N;
+  int32_t a = 0, b = N - 1;
+  for (int32_t i = 0; i < N; ++i) if (h->is_fixed[i]) { a = i; break; }
+  if (p->n_pulled > 0) b = h->pulled[0];
+  for (int32_t t = 0; t < h->T; ++t) {
+    const double *r = h->r + 3 * (size_t)N * (size_t)t;
+    double *o = o_out + 4 * (size_t)t;
+    double cm[3] = {0, 0, 0};
+    for (int32_t i = 0; i < N; ++i) for (int k = 0; k < 3; ++k) cm[k] += r[3 * (size_t)i + k];
+    for (int k = 0; k < 3; ++k) cm[k] /= (double)N;
+    double s2 = 0;
+    for (int32_t i = 0; i < N; ++i) for (int k = 0; k < 3; ++k) { double d = r[3 * (size_t)i + k] - cm[k]; s2 += d * d; }
+    o[0] = sqrt(s2 / (double)N);
+    double x2 = 0;
+    for (int k = 0; k < 3; ++k) { double d = r[3 * (size_t)b + k] - r[3 * (size_t)a + k]; x2 += d * d; }
+    o[1] = sqrt(x2);
+    double f = 0;
+    for (int32_t q = 0; q < p->n_pulled; ++q) {
+      int32_t i = h->pulled[q];
+      double proj = 0;
+      for (int k = 0; k < 3; ++k) proj += (r[3 * (size_t)i + k] - h->native[3 * (size_t)i + k]) * p->pull_dir[k];
+      f += p->pull_k * (p->pull_v * (double)h->step - proj);
+    }
+    o[2] = f;
+    double ft = 0;
+    if (p->tip_on) {
+      double c[3];
+      for (int k = 0; k < 3; ++k) c[k] = p->tip_c0[k] + p->tip_v * (double)h->step * p->tip_dir[k];
+      for (int32_t i = 0; i < N; ++i) {
+        double d[3], g2 = 0, dn = 0;
+        for (int k = 0; k < 3; ++k) { d[k] = r[3 * (size_t)i + k] - c[k]; g2 += d[k] * d[k]; dn += d[k] * p->tip_dir[k]; }
+        double g = sqrt(g2), gap = g - p->tip_R;
+        if (!(gap > 0)) return SOPO_E_NONFINITE;
+        ft += 6.0 * p->tip_eps * pow(p->tip_sigma / gap, 6.0) / gap / g * dn;
+      }
+    }
+    o[3] = ft;
+  }
+  return SOPO_OK;
+}
+
 int sopo_get_forces(sopo_handle *h, double *f_out) {
   if (!h || !f_out) return SOPO_E_ARG;
   int status = SOPO_OK;

@@ -58,6 +58,7 @@ int  sopo_set_coords(sopo_handle *, const double *xyz /*[T][N][3]*/);   /* rebui
 int  sopo_get_step(sopo_handle *, int64_t *step);
 int  sopo_set_step(sopo_handle *, int64_t step);
 int  sopo_get_energies(sopo_handle *, double *e_out /*[T][6] fene,native,rep,pull,tip,total*/);
+int  sopo_get_observables(sopo_handle *, double *o_out /*[T][4] Rg, end-to-end X, cantilever force, tip force*/);
 int  sopo_get_forces(sopo_handle *, double *f_out /*[T][N][3]*/);       /* current coords, current L2 */
 /* row counts and row contents (ascending j) of trajectory `traj`; idx is [N][cap]; cap too small -> SOPO_E_CAP */
 int  sopo_get_lists(sopo_handle *, int32_t traj, int32_t level, int32_t *row_cnt, int32_t *idx, int32_t cap,

@@ -51,6 +51,7 @@ def lib():
         L.sopo_set_step.argtypes = [C.c_void_p, C.c_int64]
         L.sopo_get_energies.argtypes = [C.c_void_p, C.c_void_p]
         L.sopo_get_forces.argtypes = [C.c_void_p, C.c_void_p]
+        L.sopo_get_observables.argtypes = [C.c_void_p, C.c_void_p]
         L.sopo_get_lists.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_int64)]
         L.sopo_max_row.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_int32)]
         L.sopo_build_lists.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32]
@@ -175,6 +176,12 @@ class Oracle:
     def get_energies(self):
         out = np.zeros((self.T, 6), np.float64)
         self._chk(lib().sopo_get_energies(self._h, out.ctypes.data), "get_energies")
+        return out
+
+    def get_observables(self):
+        """[T][4]: Rg, end-to-end distance X, cantilever force, tip force."""
+        out = np.zeros((self.T, 4), np.float64)
+        self._chk(lib().sopo_get_observables(self._h, out.ctypes.data), "get_observables")
         return out
 
     def get_forces(self):

@@ -70,6 +70,7 @@ struct sop_handle {
   int num_sms = 0;
   unsigned *S_bar = nullptr;      // grid-barrier counter of the persistent kernel
   ResDev R;                       // mode 3
+  int obs_a = 0, obs_b = 0;       // internal indices of the two ends of the end-to-end distance
   const void *res_fn = nullptr;
   uint32_t res_launch_id = 0;
   std::vector<uint32_t> tag;      // [N] host copy of the coordinate tags (internal order)
@@ -708,6 +709,8 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
     tag[ii] |= TAG_PULLED;
     adotn[ii] = (float)(X(c, 0) * nrm[0] + X(c, 1) * nrm[1] + X(c, 2) * nrm[2]);
   }
+  h->obs_a = pl.iperm[p->n_fixed > 0 ? p->fixed[0] : 0];
+  h->obs_b = pl.iperm[p->n_pulled > 0 ? p->pulled[0] : N - 1];
   std::vector<float4> pos0((size_t)N * T);
   for (int t = 0; t < T; ++t)
     for (int ii = 0; ii < N; ++ii) {
@@ -945,6 +948,18 @@ int sop_get_energies(sop_handle *h, double *e_out) {
     e[5] = e[0] + e[1] + e[2] + e[3] + e[4];
   }
   return rc;
+}
+
+int sop_get_observables(sop_handle *h, double *o_out) {
+  if (!h || !o_out) return fail(SOP_E_ARG, "null argument", h);
+  const SysDev &S = h->S;
+  double *d_o = (double *)(h->ws + h->plan.off_epart);          // reuses the energy partial buffer (>= T * 40 bytes)
+  k_observables<<<(unsigned)S.T, 1024, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, h->obs_a, h->obs_b, d_o);
+  h->launches++;
+  int rc = check_launch(h, "observables");
+  if (rc) return rc;
+  CUDA_OK(cudaMemcpyAsync(o_out, d_o, (size_t)S.T * 4 * 8, cudaMemcpyDeviceToHost, h->stream));
+  return read_flags(h);
 }
 
 int sop_get_forces(sop_handle *h, float *f_out) {

@@ -373,6 +373,66 @@ __global__ void __launch_bounds__(256) k_energy(SysDev S, int cur, unsigned long
   if (flag) atomicOr(S.flags, flag);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Observables per trajectory (PAPER.md:261 f(R) curves, :312-314 force-indentation): radius of
+// gyration, end-to-end distance between internal beads ia and ib, cantilever force summed over the pulled beads,
+// force resisting the indenter (sum_i F_i^tip . n_tip).  One block per trajectory; fp32 terms, fp64 sums, two passes
+// (centre of mass, then the squared deviations).  o_out[t][4].
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double block_sum(double v, double *red) {
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double tot = 0;
+  for (int w = 0; w < (int)(blockDim.x >> 5); ++w) tot += red[w];     // same order in every thread: deterministic
+  return tot;
+}
+
+__global__ void __launch_bounds__(1024) k_observables(SysDev S, int cur, unsigned long long step, int ia, int ib, double *o_out) {
+  __shared__ double red[32];
+  const int t = blockIdx.x;
+  const float4 *__restrict__ pos_t = S.pos[cur] + (size_t)t * S.N;
+  double sx = 0, sy = 0, sz = 0, fp = 0, ft = 0;
+  int flag = 0;
+  const float vs_pull = (float)((double)S.pull_v * (double)step), vs_tip = (float)((double)S.tip_v * (double)step);
+  const float cx = S.tip_cx + vs_tip * S.tip_nx, cy = S.tip_cy + vs_tip * S.tip_ny, cz = S.tip_cz + vs_tip * S.tip_nz;
+  for (int i = threadIdx.x; i < S.N; i += blockDim.x) {
+    const float4 r = __ldg(pos_t + i);
+    sx += (double)r.x; sy += (double)r.y; sz += (double)r.z;
+    if (S.has_pull && (__float_as_uint(r.w) & TAG_PULLED)) {
+      const float proj = r.x * S.pull_nx + r.y * S.pull_ny + r.z * S.pull_nz - __ldg(&S.pull_adotn[i]);
+      fp += (double)(S.pull_k * (vs_pull - proj));
+    }
+    if (S.tip_on) {
+      const float dx = r.x - cx, dy = r.y - cy, dz = r.z - cz;
+      const float g = sqrtf(dx * dx + dy * dy + dz * dz), gap = g - S.tip_R;
+      if (!(gap > 0.f)) flag |= FLAG_NONFINITE;
+      const float ig = 1.0f / gap, ig2 = ig * ig;
+      const float sf = 6.0f * S.tip_eps * S.tip_sigma6 * ig2 * ig2 * ig2 * ig / g;
+      ft += (double)(sf * (dx * S.tip_nx + dy * S.tip_ny + dz * S.tip_nz));
+    }
+  }
+  const double n = (double)S.N;
+  const double mx = block_sum(sx, red) / n, my = block_sum(sy, red) / n, mz = block_sum(sz, red) / n;
+  double s2 = 0;
+  for (int i = threadIdx.x; i < S.N; i += blockDim.x) {
+    const float4 r = __ldg(pos_t + i);
+    const double dx = (double)r.x - mx, dy = (double)r.y - my, dz = (double)r.z - mz;
+    s2 += dx * dx + dy * dy + dz * dz;
+  }
+  s2 = block_sum(s2, red);
+  fp = block_sum(fp, red);
+  ft = block_sum(ft, red);
+  if (threadIdx.x == 0) {
+    const float4 a = pos_t[ia], b = pos_t[ib];
+    const double dx = (double)b.x - (double)a.x, dy = (double)b.y - (double)a.y, dz = (double)b.z - (double)a.z;
+    double *o = o_out + 4 * (size_t)t;
+    o[0] = sqrt(s2 / n); o[1] = sqrt(dx * dx + dy * dy + dz * dz); o[2] = fp; o[3] = ft;
+  }
+  if (flag) atomicOr(S.flags, flag);
+}
+
 __global__ void k_energy_final(int T, int nblk, const double *partial, double *e_out) {
   int q = blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= T * 5) return;

@@ -15,7 +15,7 @@ STATUS = {0: "SOP_OK", -1: "SOP_E_ARG", -2: "SOP_E_CUDA", -3: "SOP_E_LIST_OVERFL
           -5: "SOP_E_NONFINITE"}
 
 SYMBOLS = ["sop_query_workspace", "sop_create", "sop_destroy", "sop_run", "sop_sync", "sop_get_coords",
-           "sop_set_coords", "sop_get_energies", "sop_get_forces", "sop_get_lists", "sop_get_step", "sop_set_step",
+           "sop_set_coords", "sop_get_energies", "sop_get_observables", "sop_get_forces", "sop_get_lists", "sop_get_step", "sop_set_step",
            "sop_device_coords", "sop_get_config", "sop_set_profiling", "sop_get_profile", "sop_last_error"]
 
 
@@ -69,6 +69,7 @@ def lib():
         L.sop_set_coords.argtypes = [vp, vp]
         L.sop_get_energies.argtypes = [vp, vp]
         L.sop_get_forces.argtypes = [vp, vp]
+        L.sop_get_observables.argtypes = [vp, vp]
         L.sop_get_lists.argtypes = [vp, i32, i32, vp, vp, C.POINTER(i32), C.POINTER(i64)]
         L.sop_get_step.argtypes = [vp, C.POINTER(i64)]
         L.sop_set_step.argtypes = [vp, i64]
@@ -187,6 +188,12 @@ class Sop:
         return out
 
     # -- hooks
+    def get_observables(self):
+        """[T][4] float64: Rg, end-to-end distance, cantilever force, tip force (reduced on the device)."""
+        out = np.zeros((self.T, 4), np.float64)
+        self._chk(lib().sop_get_observables(self._h, out.ctypes.data), "sop_get_observables")
+        return out
+
     def set_coords(self, xyz):
         x = np.ascontiguousarray(xyz, np.float32).reshape(self.T, self.N, 3)
         self._chk(lib().sop_set_coords(self._h, x.ctypes.data), "sop_set_coords")
@@ -253,6 +260,7 @@ def sop_get_coords(h): return h.get_coords()
 def sop_set_coords(h, xyz): return h.set_coords(xyz)
 def sop_get_energies(h): return h.get_energies()
 def sop_get_forces(h): return h.get_forces()
+def sop_get_observables(h): return h.get_observables()
 def sop_get_lists(h, level, traj=0): return h.get_lists(level, traj)
 def sop_get_step(h): return h.step
 def sop_set_step(h, v): h.step = v

@@ -402,3 +402,54 @@ def test_ensemble_means_energy_and_rg_within_3_standard_errors():
     for a, b in ((rg(xg), rg(xo)), (eg, eo)):
         se = math.sqrt(a.var(ddof=1) / T + b.var(ddof=1) / T)
         assert abs(a.mean() - b.mean()) <= 3 * se, (a.mean(), b.mean(), se)
+
+
+# ---------------------------------------------------------------------------------------------- NEXT-1: observables
+def check_observables(s, o, xg, step):
+    """device-side Rg / end-to-end distance / cantilever force / tip force == oracle at the SAME coordinates"""
+    keep, kstep = o.get_coords(), o.step
+    o.set_coords(xg.astype(np.float64)); o.step = step
+    ref = o.get_observables()
+    o.set_coords(keep); o.step = kstep
+    got = s.get_observables()
+    assert got.shape == ref.shape
+    scale = np.abs(ref) + np.array([1e-3, 1e-3, 1e-3, 1e-3])
+    assert (np.abs(got - ref) <= 2e-5 * scale + 1e-6).all(), (got, ref)     # fp32 coordinates and terms, fp64 sums
+
+
+@pytest.mark.parametrize("var", [dict(mode=1), dict(mode=3), dict(mode=3, chunk_beads=24, R_pl=20.0)], ids=str)
+def test_observables_small_with_pull_and_tip(var):
+    var = dict(var)
+    w = gen.tiny(64, 8)
+    zmax = float(w.xyz[:, 2].max())
+    p = dict(w.params, fixed=[0, 5], pulled=[63, 20], pull_k=0.05, pull_v=1e-3, pull_dir=[0.6, 0.0, 0.8],
+             tip_on=1, tip_R=50.0, tip_eps=1.0, tip_sigma=3.8, tip_c0=[0.0, 0.0, zmax + 53.0],
+             tip_dir=[0.0, 0.0, -1.0], tip_v=1e-3)
+    if "R_pl" in var:
+        p = dict(p, R_pl=var.pop("R_pl"), pl_interval=100)
+    T = 3
+    s = sop().Sop(w.xyz, w.bonds, w.native, p, n_traj=T, **var)
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, p, n_traj=T)
+    s.step = 1000; o.step = 1000
+    x0 = np.broadcast_to(w.xyz, (T,) + w.xyz.shape).copy()
+    check_observables(s, o, x0, 1000)
+    assert s.get_observables()[0, 2] > 0 and s.get_observables()[0, 3] > 0
+    s.run(100)
+    check_observables(s, o, s.get_coords(), 1100)
+    rg = s.get_observables()[:, 0]
+    assert not np.allclose(rg[0], rg[1])                      # per trajectory
+
+
+@pytest.mark.parametrize("k", [2, 3])
+def test_observables_full_configs(k):
+    w = gen.make_config(k)
+    s = sop().from_workload(w)
+    o = sopo.from_workload(w, list_builder=1)
+    check_observables(s, o, w.xyz[None], 0)
+    s.run(100)
+    check_observables(s, o, s.get_coords(), 100)
+    obs = s.get_observables()[0]
+    if k == 2:
+        assert obs[1] > 5000.0                                 # the fiber's pulled end is ~5500 A from its fixed end
+    else:
+        assert obs[3] > 0.0                                    # the indenter already pushes on the shell

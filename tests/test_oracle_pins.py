@@ -537,3 +537,57 @@ def test_fixed_beads_do_not_move_and_bad_topology_is_rejected():
         sopo.Oracle(w.xyz, w.bonds[:, ::-1], w.native, w.params)                            # i > j
     with pytest.raises(sopo.OracleError):
         sopo.Oracle(w.xyz, w.bonds, w.native, dict(w.params, pl_interval=15))               # not a multiple
+
+
+# ---------------------------------------------------------------------------------------------- P11 (NEXT-1)
+def test_p11_observables_closed_forms():
+    """sopo_get_observables against closed forms: Rg of a straight rod and of a ring, end-to-end distance, the
+    paper's f_ext = r_f t with r_f = kappa nu_0 at zero displacement, and the tip force as the
+    derivative of V_tip with respect to the tip's advance."""
+    nob = np.zeros((0, 2), np.int32)
+    base = dict(gen.BASE_PARAMS, k_fene=0.0, eps_native=0.0, eps_rep=0.0)
+    # rod of N beads spaced d along (1, 2, 2)/3: Rg^2 = d^2 (N^2 - 1) / 12, X = (N - 1) d
+    N, d = 25, 3.8
+    u = np.array([1.0, 2.0, 2.0]) / 3.0
+    rod = (np.arange(N)[:, None] * d * u[None]).astype(np.float32)
+    o = sopo.Oracle(rod, nob, nob, base)
+    rg, x, f, ft = o.get_observables()[0]
+    r64 = rod.astype(np.float64)
+    assert rg == pytest.approx(math.sqrt(d * d * (N * N - 1) / 12.0), rel=1e-6)     # fp32 input rounding only
+    assert x == pytest.approx(np.linalg.norm(r64[-1] - r64[0]), rel=1e-14)
+    assert f == 0.0 and ft == 0.0
+    # ring of radius R: Rg = R exactly (centre of mass at the centre), X between beads 0 and N-1 = 2 R sin(pi / N)
+    N, R = 36, 20.0
+    ang = 2 * math.pi * np.arange(N) / N
+    ring = np.stack([R * np.cos(ang), R * np.sin(ang), np.full(N, 5.0)], axis=1).astype(np.float32)
+    rg, x, _, _ = sopo.Oracle(ring, nob, nob, base).get_observables()[0]
+    assert rg == pytest.approx(R, rel=1e-6)
+    assert x == pytest.approx(2 * R * math.sin(math.pi / N), rel=1e-5)
+    # cantilever: fixed bead 3 and pulled bead 17 define X; at the native position f = kappa v s = r_f t
+    p = dict(base, fixed=[3], pulled=[17], pull_k=0.05, pull_v=1e-3, pull_dir=[0.0, 0.0, 1.0])
+    o = sopo.Oracle(rod, nob, nob, p)
+    o.step = 4000
+    _, x, f, _ = o.get_observables()[0]
+    assert x == pytest.approx(np.linalg.norm(r64[17] - r64[3]), rel=1e-14)
+    kappa, v = float(np.float32(0.05)), float(np.float32(1e-3))
+    assert f == pytest.approx(kappa * v * 4000, rel=1e-14)
+    moved = r64[None].copy(); moved[0, 17, 2] += 1.25                        # the bead follows the spring by 1.25 A
+    o.set_coords(moved); o.step = 4000
+    assert o.get_observables()[0, 2] == pytest.approx(kappa * (v * 4000 - 1.25), rel=1e-12)
+    # indenter: f_tip = dV_tip / d(advance); advance = v_tip * step, central difference over +-1 step
+    w = gen.tiny(40, 2)
+    pt = dict(base, tip_on=1, tip_R=50.0, tip_eps=1.0, tip_sigma=3.8, tip_c0=[0.0, 0.0, 70.0], tip_dir=[0.0, 0.0, -1.0],
+              tip_v=1e-4)
+    o = sopo.Oracle(w.xyz, nob, nob, pt)
+    s0 = 20000
+    o.step = s0
+    ft = o.get_observables()[0, 3]
+    vt = float(np.float32(1e-4))
+    x0 = w.xyz.astype(np.float64)
+    vp = o.eval_frozen(x0, step=s0 + 1, want_forces=False)[0][4]
+    vm = o.eval_frozen(x0, step=s0 - 1, want_forces=False)[0][4]
+    assert ft > 0
+    assert ft == pytest.approx((vp - vm) / (2 * vt), rel=1e-6)
+    # and it is minus the total force the tip exerts on the beads, projected on the tip direction
+    _, fb = o.eval_frozen(x0, step=s0)
+    assert ft == pytest.approx(float(fb.sum(axis=0) @ np.array([0.0, 0.0, -1.0])), rel=1e-12)
