@@ -325,12 +325,24 @@ def main():
         "e2e": main_res.get("e2e"), "gpu_launches": main_res["launches"], "clocks": main_res.get("clocks"),
     }
     sk = main_res.get("step_kernel")
+    # dram traffic of the dominant kernel per launch, from the committed ncu --set full capture (profiles/), or null
+    traffic = traffic_src = alg_per_launch = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "r1m_traffic.json.txt")) as f:
+            tr = json.load(f).get(w.name)
+        if tr and main_res["resolved"]["mode"] == 3:
+            traffic = tr["dram_bytes_per_launch"]
+            traffic_src = f"ncu dram__bytes_read.sum + dram__bytes_write.sum of one {tr['kernel']} launch = {tr['langevin_steps_per_launch']} Langevin steps (profiles/r1m_ncu_cfg3_resident.md)"
+            alg_per_launch = (main_res["bytes"]["B_fi"] + main_res["bytes"]["B_filter"] / w.params["nb_interval"]) * w.n_beads * T * tr["langevin_steps_per_launch"]
+    except Exception:  # noqa: BLE001
+        pass
     if sk:
         line["roofline"] = {
             "bound": "hbm", "kernel": "fused force+noise+update step kernel" + (" (persistent; L2 filter inside)" if sk["includes_l2_filter"] else ""),
             "achieved": sk["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": sk["achieved_gbs"] / peak, "peak_source": peak_src,
             "frac_of_nominal_8TBs": sk["achieved_gbs"] / NOMINAL_HBM_GBS, "us_per_langevin_step": sk["us_per_langevin_step"],
-            "bytes_per_bead_step": main_res["bytes"]["B_fi"], "traffic": None,
+            "bytes_per_bead_step": main_res["bytes"]["B_fi"], "traffic": traffic, "traffic_source": traffic_src,
+            "algorithmic_bytes_per_launch": alg_per_launch,
             "note": "algorithmic bytes / CUDA-event time of the step kernel; the working set is L2/SM resident, so dram traffic is far below the algorithmic bytes (profiles/)"}
     line["whole_step_gbs"] = main_res["bytes"]["B_step"] * w.n_beads * T * world / (main_res["us_per_langevin_step"] * 1e-6) / 1e9
 
