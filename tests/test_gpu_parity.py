@@ -453,3 +453,30 @@ def test_observables_full_configs(k):
         assert obs[1] > 5000.0                                 # the fiber's pulled end is ~5500 A from its fixed end
     else:
         assert obs[3] > 0.0                                    # the indenter already pushes on the shell
+
+
+def test_mode3_is_deterministic_run_to_run():
+    """compute-sanitizer is closed on this pool, so shared-memory / exchange races are hunted by repetition: the
+    SM-resident kernel must give bit-identical coordinates, lists and energies every time, on small chunked systems
+    (many exchange partners per CTA) and on the full 30,000-bead shell with all 148 CTAs polling each other."""
+    w = gen.two_chains(150, 3, R_pl=20.0)
+    for var in (dict(chunk_beads=30, lanes_per_bead=8), dict(chunk_beads=75, lanes_per_bead=1), dict(n_traj=3, chunk_beads=50)):
+        var = dict(var); T = var.pop("n_traj", 1)
+        ref = None
+        for rep in range(4):
+            s = sop().from_workload(w, n_traj=T, mode=3, **var); s.run(230)
+            out = (s.get_coords(), s.get_lists(2, T - 1)[0], s.get_energies())
+            s.close()
+            if ref is None:
+                ref = out
+            else:
+                assert all(np.array_equal(a, b) for a, b in zip(ref, out)), (var, rep)
+    w = gen.make_config(3)
+    ref = None
+    for rep in range(3):
+        s = sop().from_workload(w); s.run(200)
+        x = s.get_coords(); s.close()
+        if ref is None:
+            ref = x
+        else:
+            assert np.array_equal(ref, x), rep
