@@ -33,7 +33,7 @@ struct ResDev {
   unsigned short *pl_loc;     // [T*N][cap_pl]   L1 rows as slots
   int2 *nat_pack;             // [T][nat_entries] {slot, bits(r0^2)}   (C > 1; with one chunk slot = bead index)
   int2 *bond_pack;            // [T*N][cap_b]     {slot or -1, bits(r0)} (C > 1)
-  uint4 *xch;                 // [2][T*N][2]  {x, stamp, y, stamp} {z, stamp, -, -}
+  uint4 *xch;                 // [2][T*N][2]  {x, stamp, y, stamp, z, stamp, -, -}: one 32-byte slot per bead
   // shared-memory carve-up (bytes from the start of dynamic shared memory), computed by the host
   int off_pos, off_g, off_carry, off_tag, off_facc, off_nb, off_cnt, off_rofs, off_plcnt, off_plofs, off_pl, off_natq,
       off_nat, off_bond, off_active, off_bm, off_sbm, off_misc;
@@ -50,18 +50,20 @@ __device__ __forceinline__ float fast_rcp(float x) {
   return y;
 }
 
+// One 32-byte exchange slot per bead: {x, stamp, y, stamp, z, stamp, -, -}, written and read with ONE 256-bit access
+// (sm_100: LDG/STG.256) at gpu scope -- one L2 sector request per bead per poll instead of two.  Correctness only needs
+// each 8-byte {value, stamp} pair to be single-copy atomic (64-bit accesses are), so all three stamps are checked.
 __device__ __forceinline__ void xch_put(uint4 *slot, const float4 &v, uint32_t st) {
-  asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(slot), "r"(__float_as_uint(v.x)), "r"(st),
-               "r"(__float_as_uint(v.y)), "r"(st) : "memory");
-  asm volatile("st.volatile.global.v2.u32 [%0], {%1, %2};" ::"l"(slot + 1), "r"(__float_as_uint(v.z)), "r"(st) : "memory");
+  asm volatile("st.relaxed.gpu.global.v8.u32 [%0], {%1, %2, %3, %2, %4, %2, %5, %5};" ::"l"(slot), "r"(__float_as_uint(v.x)),
+               "r"(st), "r"(__float_as_uint(v.y)), "r"(__float_as_uint(v.z)), "r"(0u) : "memory");
 }
 
 __device__ __forceinline__ bool xch_try(const uint4 *slot, uint32_t st, float4 &out) {
-  uint32_t a0, a1, a2, a3, b0, b1;
-  asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3) : "l"(slot) : "memory");
-  asm volatile("ld.volatile.global.v2.u32 {%0, %1}, [%2];" : "=r"(b0), "=r"(b1) : "l"(slot + 1) : "memory");
-  out = make_float4(__uint_as_float(a0), __uint_as_float(a2), __uint_as_float(b0), 0.f);
-  return a1 == st && a3 == st && b1 == st;
+  uint32_t a0, a1, a2, a3, a4, a5, a6, a7;
+  asm volatile("ld.relaxed.gpu.global.v8.u32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3), "=r"(a4), "=r"(a5), "=r"(a6), "=r"(a7) : "l"(slot) : "memory");
+  out = make_float4(__uint_as_float(a0), __uint_as_float(a2), __uint_as_float(a4), 0.f);
+  return a1 == st && a3 == st && a5 == st;
 }
 
 // ------------------------------------------------------------------------------------------------
