@@ -37,7 +37,7 @@ struct Plan {                     // everything that depends only on (topology, 
   // mode 3 (SM-resident kernel): chunking, launch shape, shared-memory carve-up, workspace
   bool res_ok = false;
   std::string res_why;
-  int res_lanes = 1, res_block = 1024;
+  int res_lanes = 1, res_block = 1024, res_nat_rows = 0;
   ResDev R;
   size_t off_nhalo, off_hgid, off_plloc, off_natloc, off_bondloc, off_xch;
 };
@@ -247,6 +247,14 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
   }
   if (o > 232448 && !pl.static_l1) carve(false, 0);
   if (o > 232448) { pl.res_why = "chunk state does not fit the 227 KB of shared memory of an SM"; return; }
+  R.nat_tpad = 0;
+  pl.res_nat_rows = 0;
+  if (C == 1 && !R.nat_smem && G == 1) {          // natives stay in global memory: read them coalesced
+    std::vector<int> deg(N, 0);
+    for (int c2 = 0; c2 < tp->n_native; ++c2) { deg[tp->native[2 * c2]]++; deg[tp->native[2 * c2 + 1]]++; }
+    pl.res_nat_rows = std::max(1, *std::max_element(deg.begin(), deg.end()));
+    R.nat_tpad = (N + 31) / 32 * 32;
+  }
   if ((size_t)((N + 31) / 32) * 8 > 200000) { pl.res_why = "n_beads too large for the localise bitmap"; return; }
   if (getenv("SOP_DEBUG_PLAN"))
     fprintf(stderr, "[sop plan] mode 3: C=%d chunk=%d lanes=%d block=%d halo_cap=%d cap_nb=%d cap_pl=%d nat_smem=%d pl_cap=%d smem=%d B\n",
@@ -383,7 +391,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
     pl.off_nhalo = take((size_t)T * R.C * 4);
     pl.off_hgid = take((size_t)T * R.C * R.halo_cap * 4);
     pl.off_plloc = take(R.implicit_l1 ? 0 : I * pl.cap_pl * 2);
-    pl.off_natloc = take(multi ? (size_t)T * pl.n_nat_entries * 8 : 0);
+    pl.off_natloc = take(multi ? (size_t)T * pl.n_nat_entries * 8 : (size_t)pl.res_nat_rows * R.nat_tpad * 8);
     pl.off_bondloc = take(multi ? I * pl.cap_b * 8 : 0);
     pl.off_xch = take(multi ? 2 * I * 32 : 0);
   }
@@ -559,6 +567,11 @@ int resident_prepare(sop_handle *h) {
   R.n_halo = (int *)(w + pl.off_nhalo); R.halo_gid = (int *)(w + pl.off_hgid);
   R.pl_loc = (unsigned short *)(w + pl.off_plloc); R.nat_pack = (int2 *)(w + pl.off_natloc);
   R.bond_pack = (int2 *)(w + pl.off_bondloc); R.xch = (uint4 *)(w + pl.off_xch);
+  R.nat_T = nullptr;
+  if (R.nat_tpad > 0) {
+    R.nat_T = (int2 *)(w + pl.off_natloc);
+    k_transpose_nat<<<(h->S.N + 255) / 256, 256, 0, h->stream>>>(h->S, R);
+  }
   h->res_fn = resident_kernel(pl.res_lanes, pl.comp);
   CUDA_OK(cudaFuncSetAttribute(h->res_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, R.smem_bytes));
   const int loc_smem = ((h->S.N + 31) / 32) * 8 + R.chunk * 4;

@@ -33,6 +33,8 @@ struct ResDev {
   unsigned short *pl_loc;     // [T*N][cap_pl]   L1 rows as slots
   int2 *nat_pack;             // [T][nat_entries] {slot, bits(r0^2)}   (C > 1; with one chunk slot = bead index)
   int2 *bond_pack;            // [T*N][cap_b]     {slot or -1, bits(r0)} (C > 1)
+  int2 *nat_T;                // one chunk, natives not in shared memory: the native table transposed, entry k of bead i
+  int nat_tpad;               // at [k * nat_tpad + i], so that a warp of consecutive beads reads 256 contiguous bytes
   uint4 *xch;                 // [2][T*N][2]  {x, stamp, y, stamp, z, stamp, -, -}: one 32-byte slot per bead
   // shared-memory carve-up (bytes from the start of dynamic shared memory), computed by the host
   int off_pos, off_g, off_carry, off_tag, off_facc, off_nb, off_cnt, off_rofs, off_plcnt, off_plofs, off_pl, off_natq,
@@ -62,6 +64,7 @@ __device__ __forceinline__ bool xch_try(const uint4 *slot, uint32_t st, float4 &
   uint32_t a0, a1, a2, a3, a4, a5, a6, a7;
   asm volatile("ld.relaxed.gpu.global.v8.u32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3), "=r"(a4), "=r"(a5), "=r"(a6), "=r"(a7) : "l"(slot) : "memory");
+  (void)a6; (void)a7;
   out = make_float4(__uint_as_float(a0), __uint_as_float(a2), __uint_as_float(a4), 0.f);
   return a1 == st && a3 == st && a5 == st;
 }
@@ -169,6 +172,14 @@ __global__ void __launch_bounds__(1024) k_localise(SysDev S, ResDev R) {
       R.bond_pack[g0 * cap_b + e] = make_int2(en.x >= 0 ? slot_of(en.x) : -1, en.y);
     }
   }
+}
+
+// native table -> transposed copy (one chunk per trajectory: slot = bead index), once at create
+__global__ void k_transpose_nat(SysDev S, ResDev R) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= S.N) return;
+  const int q0 = S.nat_ptr[i], q1 = S.nat_ptr[i + 1];
+  for (int q = q0; q < q1; ++q) R.nat_T[(size_t)(q - q0) * R.nat_tpad + i] = S.nat_tab[q];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -614,8 +625,9 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         const int q1 = natq[il + 1];
         auto natives = [&](auto has_eps_t) {
           constexpr bool HAS_EPS = decltype(has_eps_t)::value;
-          for (int q = natq[il] + lane; q < q1; q += G) {
-            const int2 en = natp[q];
+          const int q0 = natq[il];
+          for (int q = q0 + lane; q < q1; q += G) {
+            const int2 en = R.nat_T ? __ldg(&R.nat_T[(size_t)(q - q0) * R.nat_tpad + il]) : natp[q];
             float e12 = K.eps12;
             if (HAS_EPS) e12 = 12.0f * __ldg(&nat_eps[q]);
             const float4 rj = pc[en.x];
