@@ -218,10 +218,9 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
     R.off_g = take(G > 1 ? 2 * (size_t)chunk * 16 : 0);
     R.off_carry = take(pl.comp ? (size_t)chunk * 16 : 0);
     R.off_tag = take((size_t)chunk * 4);
-    R.off_facc = take((size_t)chunk * 16);
+    R.off_force = take((size_t)chunk * 16);
     R.off_nb = take((size_t)chunk * R.nb_si * 2);
     R.off_cnt = take((size_t)chunk * 2);
-    R.off_rofs = take(((size_t)chunk + 1) * 4);
     R.off_plcnt = take((size_t)chunk * 2);
     R.off_plofs = take(((size_t)chunk + 1) * 4);
     R.off_pl = take((size_t)pl_cap * 2);

@@ -37,10 +37,10 @@ struct ResDev {
   int nat_tpad;               // at [k * nat_tpad + i], so that a warp of consecutive beads reads 256 contiguous bytes
   uint4 *xch;                 // [2][T*N][2]  {x, stamp, y, stamp, z, stamp, -, -}: one 32-byte slot per bead
   // shared-memory carve-up (bytes from the start of dynamic shared memory), computed by the host
-  int off_pos, off_g, off_carry, off_tag, off_facc, off_nb, off_cnt, off_rofs, off_plcnt, off_plofs, off_pl, off_natq,
+  int off_pos, off_g, off_carry, off_tag, off_force, off_nb, off_cnt, off_plcnt, off_plofs, off_pl, off_natq,
       off_nat, off_bond, off_active, off_bm, off_sbm, off_misc;
   int nb_si;                  // L2 row i starts at nb[i * nb_si] (an odd number of 32-bit words: conflict-free)
-  int nat_smem;               // the chunk's native table is copied to shared memory (nat_cap entries fit)
+  int nat_smem;               // the chunk's native table is copied to shared memory (its nat_cap entries fit)
   int nat_cap;                // largest number of native entries of a chunk
   int pl_cap;                 // 16-bit entries of shared memory for the chunk's L1 rows (0: read them from global)
   int smem_bytes;
@@ -212,13 +212,12 @@ __device__ __forceinline__ int lower_bound_dev(const int *__restrict__ a, int n,
 // k_resident: a3 + a4..a9 for n_steps Langevin steps of one chunk per CTA (see the header of this file).
 // Per step:
 //   (b) fetch the active halo of this step's layer (poll the stamps)                    -- __syncthreads --
-//   (d1) a4..a6: the chunk's bonds, native entries and L2 entries are each dealt out evenly to ALL threads as
-//        contiguous runs (a thread walks its run row by row, sums in registers, adds once per row into the per-bead
-//        fixed-point accumulators)                                                       -- __syncthreads --
+//   (d1) a4..a6 internal force, G lanes per bead: bonds, natives and the L2 row (two slots per 32-bit word) are
+//        gathered from shared memory only, lane partial sums meet by shuffle, lane 0 stores the force -- __syncthreads --
 //   (d2) a7 + a9 thread per bead: external force, update, publish; meanwhile the threads at the other end of the block
 //        generate the noise (a8) of the NEXT step, off the critical path
 //   (e) every nb_interval steps: fetch the whole halo of the new layer, Alg. 3 on the own rows (L1 rows resident in
-//        shared memory), new active set, new row offsets.
+//        shared memory when they fit), new active set.
 // Coordinates and noise are double-buffered on the step parity.
 // ------------------------------------------------------------------------------------------------
 template <int G, bool COMP>
@@ -231,7 +230,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   float4 *sg = (float4 *)(smem_raw + R.off_g);                       // [2][chunk]
   float4 *scarry = (float4 *)(smem_raw + R.off_carry);               // [chunk]      (COMP)
   uint32_t *stag = (uint32_t *)(smem_raw + R.off_tag);               // [chunk]
-  float4 *sforce = (float4 *)(smem_raw + R.off_facc);                // [chunk] internal force of this step
+  float4 *sforce = (float4 *)(smem_raw + R.off_force);                // [chunk] internal force of this step
   unsigned short *nb = (unsigned short *)(smem_raw + R.off_nb);      // L2 rows as slots, row stride nb_si
   unsigned short *cnt_s = (unsigned short *)(smem_raw + R.off_cnt);  // [chunk] L2 row counts
   unsigned short *plcnt_s = (unsigned short *)(smem_raw + R.off_plcnt);  // [chunk] L1 row counts
@@ -242,7 +241,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   int2 *sbond = (int2 *)(smem_raw + R.off_bond);                     // [chunk][cap_b]
   unsigned short *active = (unsigned short *)(smem_raw + R.off_active);
   uint32_t *bm = (uint32_t *)(smem_raw + R.off_bm), *sbm = (uint32_t *)(smem_raw + R.off_sbm);
-  int *misc = (int *)(smem_raw + R.off_misc);                        // [0] active halo slots, [1] L1 rows are in spl
+  int *misc = (int *)(smem_raw + R.off_misc);                        // [0] active halo slots, [2..7] bounding box of the in-kernel grid
 
   const int tc = blockIdx.x, t = tc / R.C, c = tc - t * R.C;
   const int b0 = c * R.chunk, b1 = min(S.N, b0 + R.chunk), n_own = b1 - b0;
