@@ -203,14 +203,14 @@ __device__ __forceinline__ bool is_excluded(const SysDev &S, int i, int j) {
 // around the bead ((2 SPAN + 1)^2 contiguous segments, the next 32 candidates in flight while the current ones are tested), keep
 // j != i in the non-native set with pred32(R_pl); ballot + prefix-popcount compaction (row order: cells z,y,x
 // ascending, beads ascending inside a cell -- deterministic; sop_get_lists returns rows sorted by the caller's index).
-// The bead's exclusion row (bonded + native partners) is staged in shared memory for the membership test.
+// The bonded / native partners are struck in a second pass over the finished row (a handful of warp iterations with the
+// exclusion row held in lane registers) instead of a membership search per candidate, which was 30 % of the kernel.
 constexpr int EXCL_SMEM = 64;
 constexpr int CELL_SPAN = 1;            // cell edge = R_pl / CELL_SPAN, scan (2 SPAN + 1)^3 cells.  SPAN = 2 tests 42 % fewer
                                         // candidates but measured slower on cfg 3 (114 vs 89 us: 25 short segments, 8x the cells)
 __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
-  __shared__ int s_excl[8][EXCL_SMEM];
   const int w = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
   if (w >= S.n_inst) return;
   const int t = w / S.N, i = w - t * S.N;
   const float4 *__restrict__ cpos = S.cell_pos + (size_t)t * S.N;
@@ -219,8 +219,9 @@ __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
   int *dst = S.pl_idx + (size_t)w * S.cap_pl;
   const float4 ri = __ldg(S.pos[cur] + (size_t)t * S.N + i);
   const int e0 = __ldg(&S.excl_ptr[i]), ne = __ldg(&S.excl_ptr[i + 1]) - e0;
-  const bool ex_smem = ne <= EXCL_SMEM;
-  if (ex_smem) for (int k = lane; k < ne; k += 32) s_excl[wib][k] = __ldg(&S.excl_idx[e0 + k]);
+  const bool ex_reg = ne <= EXCL_SMEM;                 // exclusion row in two registers per lane (else: global search)
+  const int ex0 = lane < ne ? __ldg(&S.excl_idx[e0 + lane]) : -1;
+  const int ex1 = 32 + lane < ne ? __ldg(&S.excl_idx[e0 + 32 + lane]) : -1;
   const int3 c = cell_coords(gd, ri);
   // the (z, y) rows of cells: lane l fetches the bounds of row (l / SIDE - SPAN, l % SIDE - SPAN)
   int my_s = 0, my_e = 0;
@@ -232,13 +233,6 @@ __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
       my_s = start[c0]; my_e = start[c1 + 1];
     }
   }
-  __syncwarp();
-  auto excluded = [&](int j) -> bool {
-    if (!ex_smem) return is_excluded(S, i, j);
-    int lo = 0, hi = ne;
-    while (lo < hi) { const int mid = (lo + hi) >> 1; const int v = s_excl[wib][mid]; if (v == j) return true; if (v < j) lo = mid + 1; else hi = mid; }
-    return false;
-  };
   int n = 0;
   for (int seg = 0; seg < NSEG; ++seg) {
     const int s = __shfl_sync(0xffffffffu, my_s, seg), e = __shfl_sync(0xffffffffu, my_e, seg);
@@ -255,7 +249,7 @@ __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
         if (base + 32 * u >= e) break;
         const int q = base + 32 * u + lane;
         const int j = __float_as_int(rj[u].w);
-        const bool pass = q < e && j != i && pred32(ri, rj[u], S.R_pl2) && !excluded(j);
+        const bool pass = q < e && j != i && pred32(ri, rj[u], S.R_pl2) && (ex_reg || !is_excluded(S, i, j));
         const unsigned m = __ballot_sync(0xffffffffu, pass);
         if (pass) {
           const int slot = n + __popc(m & ((1u << lane) - 1u));
@@ -265,10 +259,25 @@ __global__ void __launch_bounds__(256) k_build_l1(SysDev S, int cur) {
       }
     }
   }
-  if (lane == 0) {
-    if (n > S.cap_pl) { atomicOr(S.flags, FLAG_PL_OVERFLOW); n = S.cap_pl; }
-    S.pl_cnt[w] = n;
+  if (n > S.cap_pl) { if (lane == 0) atomicOr(S.flags, FLAG_PL_OVERFLOW); n = S.cap_pl; }
+  if (ex_reg && ne > 0) {
+    // second pass, in place and order-preserving: the write index never passes the read index
+    __syncwarp();
+    int m2 = 0;
+    for (int base = 0; base < n; base += 32) {
+      const int p = base + lane;
+      const int j = p < n ? dst[p] : -1;
+      bool hit = false;
+      for (int k = 0; k < min(ne, 32); ++k) hit |= __shfl_sync(0xffffffffu, ex0, k) == j;
+      for (int k = 32; k < ne; ++k) hit |= __shfl_sync(0xffffffffu, ex1, k - 32) == j;
+      const bool keep = p < n && !hit;
+      const unsigned m = __ballot_sync(0xffffffffu, keep);
+      if (keep) dst[m2 + __popc(m & ((1u << lane) - 1u))] = j;
+      m2 += __popc(m);
+    }
+    n = m2;
   }
+  if (lane == 0) S.pl_cnt[w] = n;
 }
 
 // R_pl = +inf: the static all-pairs L1 (Table I's "non-native pairs"), one row per bead, shared.

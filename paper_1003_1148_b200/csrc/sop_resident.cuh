@@ -61,10 +61,9 @@ __device__ __forceinline__ void xch_put(uint4 *slot, const float4 &v, uint32_t s
 }
 
 __device__ __forceinline__ bool xch_try(const uint4 *slot, uint32_t st, float4 &out) {
-  uint32_t a0, a1, a2, a3, a4, a5, a6, a7;
+  uint32_t a0, a1, a2, a3, a4, a5, a6 = 0, a7 = 0;
   asm volatile("ld.relaxed.gpu.global.v8.u32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-               : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3), "=r"(a4), "=r"(a5), "=r"(a6), "=r"(a7) : "l"(slot) : "memory");
-  (void)a6; (void)a7;
+               : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3), "=r"(a4), "=r"(a5), "+r"(a6), "+r"(a7) : "l"(slot) : "memory");
   out = make_float4(__uint_as_float(a0), __uint_as_float(a2), __uint_as_float(a4), 0.f);
   return a1 == st && a3 == st && a5 == st;
 }
