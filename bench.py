@@ -264,6 +264,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--mode", type=int, default=0)
     ap.add_argument("--lanes", type=int, default=0)
+    ap.add_argument("--sweep4", action="store_true",
+                    help="config 4's sweep of the parallelisation variant (BASELINE.json configs[4]): lanes per bead x block size")
     args = ap.parse_args()
     K, W = args.steps, max(args.warmup, 0)
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -361,6 +363,16 @@ def main():
                                   "step_kernel_frac": r.get("step_kernel", {}).get("achieved_gbs", 0.0) / peak,
                                   "B_fi": r["bytes"]["B_fi"], **r["resolved"]}
             line["workloads"] = sweep
+        if args.sweep4:
+            # thread-per-bead (1 lane) ... warp-per-bead (32 lanes) x the paper's block sizes, mode 1
+            w4 = gen.make_config(4)
+            rows = []
+            for lanes in (1, 2, 4, 8, 32):
+                for blk in (64, 128, 256):
+                    r = measure(w4, w4.n_traj, 0, 200, 2, 3, e2e=False, overrides={"mode": 1, "lanes_per_bead": lanes, "block_size": blk})
+                    rows.append({"lanes_per_bead": lanes, "block_size": blk, "us_per_langevin_step": r["us_per_langevin_step"],
+                                 "step_kernel_us": r.get("step_kernel", {}).get("us_per_langevin_step")})
+            line["cfg4_variant_sweep"] = rows
         if not args.no_cpu:
             Tc = CPU_TRAJ.get(args.config, 1)
             n = CPU_STEPS[args.config]
