@@ -549,20 +549,28 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     if (tid == 0) misc[0] = 0;
     __syncthreads();
     if (multi) {
-      for (int il = warp; il < n_own; il += nwarps) {
+      const int r8 = tid >> 3, l8 = tid & 7, g8 = bd >> 3;               // eight lanes per (short) row
+      for (int il = r8; il < n_own; il += g8) {
         const int cnt = cnt_s[il];
-        for (int p = wlane; p < cnt; p += 32) {
-          const int h = (int)nb[(size_t)il * R.nb_si + p] - n_own;
-          if (h >= 0) atomicOr(&bm[h >> 5], 1u << (h & 31));
+        const unsigned short *row = nb + (size_t)il * R.nb_si;
+        for (int p = l8; p < cnt; p += 8) {
+          const int h = (int)row[p] - n_own;
+          if (h >= 0) {
+            const uint32_t bit = 1u << (h & 31);
+            if (!(((volatile uint32_t *)bm)[h >> 5] & bit)) atomicOr(&bm[h >> 5], bit);
+          }
         }
       }
     }
     __syncthreads();
-    for (int w = tid; w < HW; w += bd) {
-      uint32_t bits = bm[w];
-      if (bits) {
-        int at = atomicAdd(&misc[0], __popc(bits));
-        while (bits) { const int b = __ffs(bits) - 1; bits &= bits - 1; active[at++] = (unsigned short)(n_own + (w << 5) + b); }
+    // bitmap -> list: a warp per word, a lane per bit (the order of the list does not matter, only who polls what)
+    for (int w = warp; w < HW; w += nwarps) {
+      const uint32_t m = bm[w];
+      if (m) {
+        int at = 0;
+        if (wlane == 0) at = atomicAdd(&misc[0], __popc(m));
+        at = __shfl_sync(0xffffffffu, at, 0);
+        if ((m >> wlane) & 1u) active[at + __popc(m & ((1u << wlane) - 1u))] = (unsigned short)(n_own + (w << 5) + wlane);
       }
     }
     __syncthreads();
