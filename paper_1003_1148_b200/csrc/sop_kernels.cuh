@@ -84,12 +84,19 @@ __global__ void k_grid_setup(SysDev S) {
   float lo[3], ext[3];
   for (int a = 0; a < 3; ++a) { lo[a] = ord2f(bb[a]); ext[a] = fmaxf(0.f, ord2f(bb[3 + a]) - lo[a]); }
   float edge = S.cell_edge;
-  int n[3];
+  int n[3] = {1, 1, 1};
   for (;;) {
-    long long tot = 1;
-    for (int a = 0; a < 3; ++a) { n[a] = (int)floorf(ext[a] / edge) + 1; tot *= n[a]; }
-    if (tot <= S.max_cells) break;
+    // cell counts in floating point first: a structure that has blown up (the error flags say so, but the run may go
+    // on) must not overflow the integer arithmetic and index out of the grid
+    float nf[3];
+    bool ok = true;
+    for (int a = 0; a < 3; ++a) { nf[a] = floorf(ext[a] / edge) + 1.0f; ok = ok && nf[a] >= 1.0f && nf[a] < 1.0e6f; }
+    if (ok && (double)nf[0] * (double)nf[1] * (double)nf[2] <= (double)S.max_cells) {
+      for (int a = 0; a < 3; ++a) n[a] = (int)nf[a];
+      break;
+    }
     edge *= 1.25f;                       // cells may only grow: any edge >= cell_edge keeps the scan complete
+    if (!(edge < 1.0e30f)) break;        // non-finite extent: one cell
   }
   GridDev gd;
   gd.ox = lo[0]; gd.oy = lo[1]; gd.oz = lo[2];

@@ -403,11 +403,13 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
       const float ox = ord2f(misc[2]), oy = ord2f(misc[3]), oz = ord2f(misc[4]);
       const float ex = fmaxf(0.f, ord2f(misc[5]) - ox), ey = fmaxf(0.f, ord2f(misc[6]) - oy), ez = fmaxf(0.f, ord2f(misc[7]) - oz);
       float edge = sqrtf(S.R_nb2) * 1.001f;
-      int nx, ny, nz;
-      for (;;) {
-        nx = (int)floorf(ex / edge) + 1; ny = (int)floorf(ey / edge) + 1; nz = (int)floorf(ez / edge) + 1;
-        if ((long long)nx * ny * nz <= RES_GRID_CELLS) break;
+      int nx = 1, ny = 1, nz = 1;
+      for (;;) {                             // counts in floating point first: no integer overflow on a blown-up chain
+        const float fx = floorf(ex / edge) + 1.0f, fy = floorf(ey / edge) + 1.0f, fz = floorf(ez / edge) + 1.0f;
+        if (fx >= 1.0f && fy >= 1.0f && fz >= 1.0f && fx < 1.0e6f && fy < 1.0e6f && fz < 1.0e6f &&
+            (double)fx * (double)fy * (double)fz <= (double)RES_GRID_CELLS) { nx = (int)fx; ny = (int)fy; nz = (int)fz; break; }
         edge *= 1.25f;                       // cells may only grow: the 27-cell scan stays complete
+        if (!(edge < 1.0e30f)) break;        // non-finite extent: one cell
       }
       const float inv_edge = 1.0f / edge;
       const int ncell = nx * ny * nz;

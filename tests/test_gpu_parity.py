@@ -480,3 +480,28 @@ def test_mode3_is_deterministic_run_to_run():
             ref = x
         else:
             assert np.array_equal(ref, x), rep
+
+
+@pytest.mark.parametrize("var", [dict(mode=1), dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=40)], ids=str)
+def test_a_blown_up_structure_reports_errors_but_stays_memory_safe(var):
+    """A caller that ignores SOP_E_FENE / SOP_E_NONFINITE and keeps running must keep getting status codes, never a
+    CUDA fault: the cell grid of a structure with a bead at 1e30 A (or NaN) once overflowed its integer arithmetic."""
+    m = sop()
+    w = gen.tiny(160, 14, R_pl=20.0)
+    for bad in (np.float32(1.0e30), np.float32("nan"), np.float32("inf")):
+        s = m.from_workload(w, **var)
+        x = w.xyz[None].copy(); x[0, 7, 1] = bad
+        codes = []
+        try:
+            s.set_coords(x)
+        except m.SopError as e:
+            codes.append(e.code)
+        for _ in range(3):
+            try:
+                s.run(130); s.sync()
+            except m.SopError as e:
+                codes.append(e.code)
+        assert codes and all(c in (-3, -4, -5) for c in codes), codes
+        s.close()
+    # the device is still healthy
+    s = m.from_workload(w, **var); s.run(50); s.sync(); s.close()
