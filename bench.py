@@ -330,11 +330,11 @@ def main():
     # dram traffic of the dominant kernel per launch, from the committed ncu --set full capture (profiles/), or null
     traffic = traffic_src = alg_per_launch = None
     try:
-        with open(os.path.join(ROOT, "profiles", "r1n_traffic.json.txt")) as f:
+        with open(os.path.join(ROOT, "profiles", "r1p_traffic.json.txt")) as f:
             tr = json.load(f).get(w.name)
         if tr and main_res["resolved"]["mode"] == 3:
             traffic = tr["dram_bytes_per_launch"]
-            traffic_src = f"ncu dram__bytes_read.sum + dram__bytes_write.sum of one {tr['kernel']} launch = {tr['langevin_steps_per_launch']} Langevin steps (profiles/r1n_ncu_cfg3_resident.md)"
+            traffic_src = f"ncu dram__bytes_read.sum + dram__bytes_write.sum of one {tr['kernel']} launch = {tr['langevin_steps_per_launch']} Langevin steps (profiles/r1p_ncu_cfg3_resident.md)"
             alg_per_launch = (main_res["bytes"]["B_fi"] + main_res["bytes"]["B_filter"] / w.params["nb_interval"]) * w.n_beads * T * tr["langevin_steps_per_launch"]
     except Exception:  # noqa: BLE001
         pass
