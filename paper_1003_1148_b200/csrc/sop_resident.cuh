@@ -96,16 +96,17 @@ __global__ void __launch_bounds__(1024) k_localise(SysDev S, ResDev R) {
     if (j < b0 || j >= b1) { const uint32_t bit = 1u << (j & 31); if (!(((volatile uint32_t *)bm)[j >> 5] & bit)) atomicOr(&bm[j >> 5], bit); }
   };
   const int *rows = S.pl_idx + g0 * cap_pl;
-  const int n_rows_e = n_own * cap_pl;
-  for (int e0 = tid; e0 < n_rows_e; e0 += 4 * bd) {          // four independent loads in flight per thread
-    int v[4];
+  // a warp per row, four independent loads per lane in flight (no index arithmetic per entry, no padding visited)
+  for (int r = warp; r < n_own; r += nwarps) {
+    const int c_r = cnt[r];
+    const int *row = rows + (size_t)r * cap_pl;
+    for (int p0 = lane; p0 < c_r; p0 += 128) {
+      int v[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int e = e0 + u * bd, r = e / cap_pl;
-      v[u] = (e < n_rows_e && e - r * cap_pl < cnt[r]) ? rows[e] : -1;
+      for (int u = 0; u < 4; ++u) v[u] = p0 + 32 * u < c_r ? row[p0 + 32 * u] : -1;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) if (v[u] >= 0) mark(v[u]);
     }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) if (v[u] >= 0) mark(v[u]);
   }
   const int q0 = S.nat_ptr[b0], q1 = S.nat_ptr[b1];
   const bool multi = R.C > 1;
@@ -151,15 +152,17 @@ __global__ void __launch_bounds__(1024) k_localise(SysDev S, ResDev R) {
     return n_own + (int)pre[j >> 5] + __popc(bm[j >> 5] & ((1u << (j & 31)) - 1u));
   };
   unsigned short *loc = R.pl_loc + g0 * cap_pl;
-  for (int e0 = tid; e0 < n_rows_e; e0 += 4 * bd) {
-    int v[4];
+  for (int r = warp; r < n_own; r += nwarps) {
+    const int c_r = cnt[r];
+    const int *row = rows + (size_t)r * cap_pl;
+    unsigned short *lrow = loc + (size_t)r * cap_pl;
+    for (int p0 = lane; p0 < c_r; p0 += 128) {
+      int v[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int e = e0 + u * bd, r = e / cap_pl;
-      v[u] = (e < n_rows_e && e - r * cap_pl < cnt[r]) ? rows[e] : -1;
+      for (int u = 0; u < 4; ++u) v[u] = p0 + 32 * u < c_r ? row[p0 + 32 * u] : -1;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) if (v[u] >= 0) lrow[p0 + 32 * u] = (unsigned short)slot_of(v[u]);
     }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) if (v[u] >= 0) loc[e0 + u * bd] = (unsigned short)slot_of(v[u]);
   }
   if (multi) {                                  // one chunk: slot = bead index, natives and bonds need no table
     for (int q = q0 + tid; q < q1; q += bd) {
