@@ -77,12 +77,10 @@ __global__ void __launch_bounds__(256) k_bbox(SysDev S, int cur) {
   }
 }
 
-__global__ void k_grid_setup(SysDev S) {
-  int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= S.T) return;
-  const int *bb = (const int *)S.bbox + t * 6;
-  float lo[3], ext[3];
-  for (int a = 0; a < 3; ++a) { lo[a] = ord2f(bb[a]); ext[a] = fmaxf(0.f, ord2f(bb[3 + a]) - lo[a]); }
+// grid parameters from a bounding box: cells of edge >= cell_edge, grown until they fit max_cells
+__device__ __forceinline__ GridDev make_grid(const SysDev &S, const float lo[3], const float hi[3]) {
+  float ext[3];
+  for (int a = 0; a < 3; ++a) ext[a] = fmaxf(0.f, hi[a] - lo[a]);
   float edge = S.cell_edge;
   int n[3] = {1, 1, 1};
   for (;;) {
@@ -103,7 +101,16 @@ __global__ void k_grid_setup(SysDev S) {
   gd.inv_edge = 1.0f / edge;
   gd.nx = n[0]; gd.ny = n[1]; gd.nz = n[2];
   gd.ncell = n[0] * n[1] * n[2];
-  S.grid[t] = gd;
+  return gd;
+}
+
+__global__ void k_grid_setup(SysDev S) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= S.T) return;
+  const int *bb = (const int *)S.bbox + t * 6;
+  float lo[3], hi[3];
+  for (int a = 0; a < 3; ++a) { lo[a] = ord2f(bb[a]); hi[a] = ord2f(bb[3 + a]); }
+  S.grid[t] = make_grid(S, lo, hi);
 }
 
 __device__ __forceinline__ int3 cell_coords(const GridDev &gd, const float4 &r) {
