@@ -83,6 +83,10 @@ typedef struct {
   int32_t reorder;                   /* 0 auto, 1 sort beads by native position inside the library, 2 keep order;
                                         invisible at the boundary (all indices in and out are the caller's) */
   int32_t chunk_beads;               /* mode 3: beads per chunk (one chunk per CTA); 0 auto */
+  int32_t rng;                       /* 0 counter-based Philox4x32-10 (no generator state in memory); 1 the paper's Hybrid
+                                        Taus (Alg. 6): 16 bytes of state per bead instance read and
+                                        written every step, seeded from Philox(seed); modes 1 and 2 only.  The state is
+                                        not part of sop_set_coords / sop_set_step, so an exact resume needs rng = 0 */
   void *stream;                      /* cudaStream_t */
 } sop_params;
 

@@ -29,6 +29,7 @@ struct sopo_handle {
   int32_t n_native; int32_t *nat_i, *nat_j;    double *nat_r0, *nat_eps;
   sopo_params p;
   unsigned char *is_fixed;        /* [N] */
+  uint32_t *taus;                 /* [T][N][4] Hybrid Taus states (params.rng == 1) */
   int32_t *pulled;                /* [n_pulled] */
   double *native;                 /* [N][3] promoted native coordinates (anchors of the pulled beads) */
   int64_t *excl_ptr; int32_t *excl_idx;   /* bonded + native partners of each bead, ascending */
@@ -75,6 +76,48 @@ void sopo_normals(uint64_t seed, uint32_t bead, uint32_t traj, uint64_t step, do
   uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
   uint32_t x[4];
   sopo_philox4x32_10(ctr, key, x);
+  double u_a = ((double)(x[0] >> 8) + 1.0) * (1.0 / 16777216.0);
+  double u_b = ((double)(x[1] >> 8)) * (1.0 / 16777216.0);
+  double u_c = ((double)(x[2] >> 8) + 1.0) * (1.0 / 16777216.0);
+  double u_d = ((double)(x[3] >> 8)) * (1.0 / 16777216.0);
+  double ra = sqrt(-2.0 * log(u_a));
+  double rc = sqrt(-2.0 * log(u_c));
+  g_out[0] = ra * cos(TWO_PI * u_b);
+  g_out[1] = ra * sin(TWO_PI * u_b);
+  g_out[2] = rc * cos(TWO_PI * u_d);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Hybrid Taus (Alg. 6): three Tausworthe components + one LCG, four 32-bit words of state per
+ * bead ("one-PRNG-per-thread"), output = y1 ^ y2 ^ y3 ^ y4.  The listing's constants are garbled in PAPER.md:209
+ * (c21 and c31 appear twice); reading R12 takes the taus88 / GPU Gems 3 ch. 37 set the paper cites ([49]-[51]):
+ * (13, 19, 12, 4294967294), (2, 25, 4, 4294967288), (3, 11, 17, 4294967280), LCG a = 1664525, c = 1013904223.
+ * ------------------------------------------------------------------------------------------------ */
+uint32_t sopo_taus_step(uint32_t y[4]) {
+  uint32_t b;
+  b = ((y[0] << 13) ^ y[0]) >> 19;  y[0] = ((y[0] & 4294967294u) << 12) ^ b;      /* lines 6-7  */
+  b = ((y[1] << 2) ^ y[1]) >> 25;   y[1] = ((y[1] & 4294967288u) << 4) ^ b;       /* lines 8-9  */
+  b = ((y[2] << 3) ^ y[2]) >> 11;   y[2] = ((y[2] & 4294967280u) << 17) ^ b;      /* lines 10-11 */
+  y[3] = 1664525u * y[3] + 1013904223u;                                           /* line 12 */
+  return y[0] ^ y[1] ^ y[2] ^ y[3];                                               /* line 13 (before mult) */
+}
+
+/* Initial seeds of one bead's generator (Alg. 6 line 1: "initial seeds", generated on the CPU):
+ * the four words of Philox4x32-10(counter = (bead, traj, 'TAUS', 0), key = seed); the Tausworthe components need
+ * y1 >= 2, y2 >= 8, y3 >= 16 (L'Ecuyer), enforced by setting that bit. */
+void sopo_taus_seed(uint64_t seed, uint32_t bead, uint32_t traj, uint32_t y[4]) {
+  uint32_t ctr[4] = { bead, traj, 0x54415553u, 0u };
+  uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+  sopo_philox4x32_10(ctr, key, y);
+  y[0] |= 2u; y[1] |= 8u; y[2] |= 16u;
+}
+
+/* Three normals from four consecutive Hybrid Taus draws: the same 24-bit uniforms and Box-Muller as sopo_normals
+ * (the paper's mult * x can be exactly 0, whose logarithm diverges; reading R6 keeps u_a, u_c in (0, 1]). */
+static void taus_normals(uint32_t y[4], double g_out[3]) {
+  const double TWO_PI = 6.283185307179586476925286766559;
+  uint32_t x[4];
+  for (int k = 0; k < 4; ++k) x[k] = sopo_taus_step(y);
   double u_a = ((double)(x[0] >> 8) + 1.0) * (1.0 / 16777216.0);
   double u_b = ((double)(x[1] >> 8)) * (1.0 / 16777216.0);
   double u_c = ((double)(x[2] >> 8) + 1.0) * (1.0 / 16777216.0);
@@ -224,6 +267,13 @@ int sopo_create(const sopo_topology *tp, const float *native_xyz, const sopo_par
   h->p.fixed = NULL; h->p.pulled = h->pulled;
 
   h->r = (double *)malloc(sizeof(double) * 3 * (size_t)N * (size_t)n_traj);
+  h->taus = NULL;
+  if (p->rng == 1) {
+    h->taus = (uint32_t *)malloc(sizeof(uint32_t) * 4 * (size_t)N * (size_t)n_traj);
+    for (int32_t t = 0; t < n_traj; ++t)
+      for (int32_t i = 0; i < N; ++i)
+        sopo_taus_seed(p->seed, (uint32_t)i, (uint32_t)(p->traj_offset + t), h->taus + 4 * ((size_t)N * (size_t)t + (size_t)i));
+  }
   h->L1 = (csr_t *)calloc((size_t)n_traj, sizeof(csr_t));
   h->L2 = (csr_t *)calloc((size_t)n_traj, sizeof(csr_t));
   h->static_l1 = isinf(p->R_pl) ? 1 : 0;
@@ -242,7 +292,7 @@ void sopo_destroy(sopo_handle *h) {
   if (!h) return;
   free(h->bond_i); free(h->bond_j); free(h->bond_r0);
   free(h->nat_i); free(h->nat_j); free(h->nat_r0); free(h->nat_eps);
-  free(h->is_fixed); free(h->pulled); free(h->native); free(h->excl_ptr); free(h->excl_idx); free(h->r);
+  free(h->taus); free(h->is_fixed); free(h->pulled); free(h->native); free(h->excl_ptr); free(h->excl_idx); free(h->r);
   if (h->L1) for (int32_t t = 0; t < h->T; ++t) csr_free(&h->L1[t]);
   if (h->L2) for (int32_t t = 0; t < h->T; ++t) csr_free(&h->L2[t]);
   free(h->L1); free(h->L2);
@@ -517,7 +567,8 @@ static int step_one(sopo_handle *h, int32_t t, int64_t step, double *fbuf) {
   for (int32_t i = 0; i < N; ++i) {
     if (h->is_fixed[i]) continue;
     double g[3];
-    sopo_normals(h->p.seed, (uint32_t)i, (uint32_t)(h->p.traj_offset + t), (uint64_t)step, g);
+    if (h->p.rng == 1) taus_normals(h->taus + 4 * ((size_t)N * (size_t)t + (size_t)i), g);   /* state read, 4 draws, state written back */
+    else sopo_normals(h->p.seed, (uint32_t)i, (uint32_t)(h->p.traj_offset + t), (uint64_t)step, g);
     for (int a = 0; a < 3; ++a) {
       double v = r[3 * (size_t)i + a] + D * fbuf[3 * (size_t)i + a] + amp * g[a];
       if (!isfinite(v)) status = status ? status : SOPO_E_NONFINITE;

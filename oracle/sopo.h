@@ -45,6 +45,8 @@ typedef struct {
   int32_t tip_on; double tip_R, tip_eps, tip_sigma, tip_c0[3], tip_dir[3], tip_v;
   int32_t list_builder;                        /* 0 brute force over all j (the definition); 1 the oracle's own
                                                   cell list (tests prove it equal to 0; used for big N only) */
+  int32_t rng;                                 /* 0 counter-based Philox (reading R6); 1 the paper's Hybrid Taus
+                                                  (Alg. 6), state per bead, reading R12 */
 } sopo_params;
 
 enum { SOPO_OK = 0, SOPO_E_ARG = -1, SOPO_E_CAP = -3, SOPO_E_FENE = -4, SOPO_E_NONFINITE = -5 };
@@ -58,6 +60,8 @@ int  sopo_set_coords(sopo_handle *, const double *xyz /*[T][N][3]*/);   /* rebui
 int  sopo_get_step(sopo_handle *, int64_t *step);
 int  sopo_set_step(sopo_handle *, int64_t step);
 int  sopo_get_energies(sopo_handle *, double *e_out /*[T][6] fene,native,rep,pull,tip,total*/);
+uint32_t sopo_taus_step(uint32_t y[4]);       /* one Hybrid Taus draw; advances the state */
+void sopo_taus_seed(uint64_t seed, uint32_t bead, uint32_t traj, uint32_t y[4]);
 int  sopo_get_observables(sopo_handle *, double *o_out /*[T][4] Rg, end-to-end X, cantilever force, tip force*/);
 int  sopo_get_forces(sopo_handle *, double *f_out /*[T][N][3]*/);       /* current coords, current L2 */
 /* row counts and row contents (ascending j) of trajectory `traj`; idx is [N][cap]; cap too small -> SOPO_E_CAP */

@@ -34,7 +34,7 @@ class _Params(C.Structure):
                 ("pull_k", C.c_double), ("pull_v", C.c_double), ("pull_dir", C.c_double * 3),
                 ("tip_on", C.c_int32), ("tip_R", C.c_double), ("tip_eps", C.c_double), ("tip_sigma", C.c_double),
                 ("tip_c0", C.c_double * 3), ("tip_dir", C.c_double * 3), ("tip_v", C.c_double),
-                ("list_builder", C.c_int32)]
+                ("list_builder", C.c_int32), ("rng", C.c_int32)]
 
 
 def lib():
@@ -52,6 +52,10 @@ def lib():
         L.sopo_get_energies.argtypes = [C.c_void_p, C.c_void_p]
         L.sopo_get_forces.argtypes = [C.c_void_p, C.c_void_p]
         L.sopo_get_observables.argtypes = [C.c_void_p, C.c_void_p]
+        L.sopo_taus_step.argtypes = [C.c_void_p]
+        L.sopo_taus_step.restype = C.c_uint32
+        L.sopo_taus_seed.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
+        L.sopo_taus_seed.restype = None
         L.sopo_get_lists.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_int64)]
         L.sopo_max_row.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_int32)]
         L.sopo_build_lists.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32]
@@ -137,6 +141,7 @@ class Oracle:
         pp.tip_dir = (C.c_double * 3)(*[f32(v) for v in p.get("tip_dir", [0, 0, -1])])
         pp.tip_v = f32(p.get("tip_v", 0.0))
         pp.list_builder = int(list_builder)
+        pp.rng = int(p.get("rng", 0))
         self._h = C.c_void_p()
         rc = L.sopo_create(C.byref(tp), self._xyz.ctypes.data, C.byref(pp), self.T, C.byref(self._h))
         if rc:
@@ -231,3 +236,14 @@ class Oracle:
 
 def from_workload(w, n_traj=None, **kw):
     return Oracle(w.xyz, w.bonds, w.native, w.params, n_traj=w.n_traj if n_traj is None else n_traj, **kw)
+
+
+def taus_step(y):
+    """One Hybrid Taus draw (Alg. 6): y = 4 uint32 words of state, advanced in place; returns the 32-bit output."""
+    return int(lib().sopo_taus_step(y.ctypes.data))
+
+
+def taus_seed(seed, bead, traj):
+    y = np.zeros(4, np.uint32)
+    lib().sopo_taus_seed(int(seed), int(bead), int(traj), y.ctypes.data)
+    return y

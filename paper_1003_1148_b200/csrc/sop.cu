@@ -33,7 +33,7 @@ struct Plan {                     // everything that depends only on (topology, 
   // workspace offsets
   size_t off_pos0, off_pos1, off_carry, off_force, off_bond, off_natptr, off_nattab, off_nateps, off_exclptr,
       off_exclidx, off_adotn, off_plcnt, off_plidx, off_nbcnt, off_nbidx, off_bbox, off_grid, off_cellof,
-      off_cellcnt, off_cellstart, off_cellbead, off_cellpos, off_flags, off_epart, off_eout, off_bar, total;
+      off_cellcnt, off_cellstart, off_cellbead, off_cellpos, off_taus, off_flags, off_epart, off_eout, off_bar, total;
   // mode 3 (SM-resident kernel): chunking, launch shape, shared-memory carve-up, workspace
   bool res_ok = false;
   std::string res_why;
@@ -348,7 +348,10 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.block = p->block_size > 0 ? p->block_size : 256;
   if (pl.block % 32 || pl.block > 1024) return fail(SOP_E_ARG, "block_size must be a multiple of 32, <= 1024");
   if (p->mode < 0 || p->mode > 3) return fail(SOP_E_ARG, "mode must be 0, 1, 2 or 3");
+  if (p->rng != 0 && p->rng != 1) return fail(SOP_E_ARG, "rng must be 0 (Philox) or 1 (Hybrid Taus)");
+  if (p->rng == 1 && p->mode == 3) return fail(SOP_E_ARG, "rng = 1 (Hybrid Taus) runs in modes 1 and 2 only");
   pl.mode = p->mode;
+  if (p->rng == 1 && pl.mode == 0) pl.mode = inst > 100000 ? 1 : 2;
   if (pl.mode == 0 || pl.mode == 3) {
     plan_resident(tp, p, x, pl);
     if (pl.mode == 3 && !pl.res_ok) return fail(SOP_E_ARG, "mode 3 is not possible here: " + pl.res_why);
@@ -380,6 +383,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.off_cellstart = take(pl.static_l1 ? 0 : (size_t)T * ((size_t)pl.max_cells + 1) * 4);
   pl.off_cellbead = take(pl.static_l1 ? 0 : I * 4);
   pl.off_cellpos = take(pl.static_l1 ? 0 : I * 16);
+  pl.off_taus = take(p->rng == 1 ? I * 16 : 0);
   pl.off_flags = take(64);
   pl.off_epart = take((size_t)T * pl.energy_blocks * 5 * 8);
   pl.off_eout = take((size_t)T * 6 * 8);
@@ -768,6 +772,7 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
   S.tip_sigma6 = (float)std::pow((double)p->tip_sigma, 6.0); S.tip_v = p->tip_v;
   S.tip_cx = p->tip_c0[0]; S.tip_cy = p->tip_c0[1]; S.tip_cz = p->tip_c0[2];
   S.tip_nx = p->tip_dir[0]; S.tip_ny = p->tip_dir[1]; S.tip_nz = p->tip_dir[2];
+  S.taus = p->rng == 1 ? (uint4 *)(w + pl.off_taus) : nullptr;
   S.flags = (int *)(w + pl.off_flags);
 
   // ---- upload (synchronous copies from pageable host vectors; create is not on the hot path)
@@ -807,6 +812,10 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
     if (rc) { std::string m = g_last_error; delete h; return fail(rc, m); }
   }
 
+  if (S.taus) {
+    k_taus_seed<<<(unsigned)((S.n_inst + 255) / 256), 256, 0, h->stream>>>(S, 0);
+    h->launches++;
+  }
   h->cur = 0; h->step = 0;
   rc = rebuild_lists(h);
   if (!rc) rc = read_flags(h);

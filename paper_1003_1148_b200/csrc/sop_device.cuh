@@ -64,6 +64,7 @@ struct SysDev {
   int traj_offset;
   int has_pull; float pull_k, pull_v, pull_nx, pull_ny, pull_nz;
   int tip_on; float tip_R, tip_eps, tip_sigma6, tip_v, tip_cx, tip_cy, tip_cz, tip_nx, tip_ny, tip_nz;
+  uint4 *taus;                      // [T][N] Hybrid Taus states (params.rng == 1), else nullptr
   int *flags;
 };
 
@@ -233,6 +234,36 @@ __device__ __forceinline__ void external_force(const SysDev &S, int i, const flo
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// NEXT-2: the paper's Hybrid Taus generator (Alg. 6; constants: DESIGN.md reading R12): three
+// Tausworthe components and one LCG, 16 bytes of state per bead instance in global memory, four draws per bead-step.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t taus_draw(uint4 &y) {
+  uint32_t b;
+  b = ((y.x << 13) ^ y.x) >> 19;  y.x = ((y.x & 4294967294u) << 12) ^ b;
+  b = ((y.y << 2) ^ y.y) >> 25;   y.y = ((y.y & 4294967288u) << 4) ^ b;
+  b = ((y.z << 3) ^ y.z) >> 11;   y.z = ((y.z & 4294967280u) << 17) ^ b;
+  y.w = 1664525u * y.w + 1013904223u;
+  return y.x ^ y.y ^ y.z ^ y.w;
+}
+
+__device__ __forceinline__ float3 box_muller3(uint32_t x0, uint32_t x1, uint32_t x2, uint32_t x3) {
+  const float k = 1.0f / 16777216.0f;
+  float ua = (float)((x0 >> 8) + 1u) * k, ub = (float)(x1 >> 8) * k, uc = (float)((x2 >> 8) + 1u) * k, ud = (float)(x3 >> 8) * k;
+  float ra = sqrtf(-2.0f * __logf(ua)), rc = sqrtf(-2.0f * __logf(uc));
+  float sb, cb;
+  __sincosf(6.283185307179586f * ub, &sb, &cb);
+  return make_float3(ra * cb, ra * sb, rc * __cosf(6.283185307179586f * ud));
+}
+
+// state load, four draws, state store: the traffic the counter-based generator does not have
+__device__ __forceinline__ float3 gaussian3_taus(uint4 *state) {
+  uint4 y = *state;
+  const uint32_t x0 = taus_draw(y), x1 = taus_draw(y), x2 = taus_draw(y), x3 = taus_draw(y);
+  *state = y;
+  return box_muller3(x0, x1, x2, x3);
+}
+
 // a9: the position update of Alg. 7 line 5 given the three normals, optionally Kahan-compensated (R10).
 template <bool COMP>
 __device__ __forceinline__ float4 langevin_apply(const SysDev &S, const float4 &ri, const float3 &gn, float fx, float fy,
@@ -259,9 +290,9 @@ __device__ __forceinline__ float4 langevin_apply(const SysDev &S, const float4 &
 template <bool COMP>
 __device__ __forceinline__ float4 langevin_update(const SysDev &S, const float4 &ri, uint32_t tag, int t,
                                                   unsigned long long step, float fx, float fy, float fz,
-                                                  float4 *carry_slot, int &flag) {
+                                                  float4 *carry_slot, int &flag, int inst = 0) {
   if (tag & TAG_FIXED) return ri;                                     // fixed beads are copied unchanged
-  float3 gn = gaussian3(S, tag & TAG_ID_MASK, (uint32_t)(S.traj_offset + t), step);
+  float3 gn = S.taus ? gaussian3_taus(S.taus + inst) : gaussian3(S, tag & TAG_ID_MASK, (uint32_t)(S.traj_offset + t), step);
   return langevin_apply<COMP>(S, ri, gn, fx, fy, fz, carry_slot, flag);
 }
 

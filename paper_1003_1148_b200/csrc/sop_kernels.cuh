@@ -27,10 +27,21 @@ __global__ void __launch_bounds__(1024) k_step(SysDev S, int cur, unsigned long 
     if (FORCES) {
       S.force[gg] = make_float4(f.x, f.y, f.z, 0.f);
     } else {
-      S.pos[cur ^ 1][gg] = langevin_update<COMP>(S, ri, tag, t, step, f.x, f.y, f.z, COMP ? S.carry + gg : nullptr, flag);
+      S.pos[cur ^ 1][gg] = langevin_update<COMP>(S, ri, tag, t, step, f.x, f.y, f.z, COMP ? S.carry + gg : nullptr, flag, gg);
     }
   }
   if (flag) atomicOr(S.flags, flag);
+}
+
+// initial Hybrid Taus states (Alg. 6 line 1): Philox4x32-10(counter = (bead, traj, 'TAUS', 0), key = seed), with the
+// bits that keep the Tausworthe components off their degenerate states (y1 >= 2, y2 >= 8, y3 >= 16)
+__global__ void k_taus_seed(SysDev S, int cur) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= S.n_inst) return;
+  const uint32_t bead = __float_as_uint(S.pos[cur][g].w) & TAG_ID_MASK;
+  uint4 y = philox4x32_10(make_uint4(bead, (uint32_t)(S.traj_offset + g / S.N), 0x54415553u, 0u), make_uint2(S.seed_lo, S.seed_hi));
+  y.x |= 2u; y.y |= 8u; y.z |= 16u;
+  S.taus[g] = y;
 }
 
 // a3: L2 neighbor-list filter (Alg. 3), one warp per bead instance.

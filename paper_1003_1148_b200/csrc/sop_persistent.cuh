@@ -47,7 +47,7 @@ __global__ void __launch_bounds__(1024) k_persist(SysDev S, int cur, unsigned lo
       if (valid && lane == 0) {
         const uint32_t tag = __float_as_uint(ri.w);
         external_force(S, i, ri, tag, step, f.x, f.y, f.z, flag);
-        pout[gg] = langevin_update<COMP>(S, ri, tag, t, step, f.x, f.y, f.z, COMP ? S.carry + gg : nullptr, flag);
+        pout[gg] = langevin_update<COMP>(S, ri, tag, t, step, f.x, f.y, f.z, COMP ? S.carry + gg : nullptr, flag, gg);
       }
     }
     grid_barrier(bar, (unsigned)(s + 1) * gridDim.x);

@@ -505,3 +505,30 @@ def test_a_blown_up_structure_reports_errors_but_stays_memory_safe(var):
         s.close()
     # the device is still healthy
     s = m.from_workload(w, **var); s.run(50); s.sync(); s.close()
+
+
+# ---------------------------------------------------------------------------------------------- NEXT-2: Hybrid Taus
+@pytest.mark.parametrize("var", [dict(mode=1, lanes_per_bead=4), dict(mode=2), dict(mode=0), dict(mode=1, reorder=1)], ids=str)
+def test_hybrid_taus_noise_matches_the_oracle(var):
+    """params.rng = 1: the paper's per-bead Hybrid Taus generator (Alg. 6).  Same seeds, same state stream per bead on
+    both sides -> coordinates within 1e-3 A after 100 steps; fixed beads draw nothing; run splits do not matter."""
+    m = sop()
+    w = gen.two_chains(120, 5, R_pl=20.0)
+    p = dict(w.params, rng=1, fixed=[0, 7])
+    T = 3
+    s = m.Sop(w.xyz, w.bonds, w.native, p, n_traj=T, **var)
+    assert s.config()["mode"] in (1, 2)
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, p, n_traj=T)
+    s.run(100); o.run(100)
+    xg, xo = s.get_coords(), o.get_coords()
+    assert np.abs(xg - xo).max() <= 1e-3
+    assert not np.array_equal(xg[0], xg[1])
+    assert np.array_equal(xg[0, 0], w.xyz[0]) and np.array_equal(xg[2, 7], w.xyz[7])
+    b = m.Sop(w.xyz, w.bonds, w.native, p, n_traj=T, **var); b.run(37); b.run(63)
+    assert np.array_equal(b.get_coords(), xg)
+    # a different generator than Philox, same physics
+    c = m.Sop(w.xyz, w.bonds, w.native, dict(p, rng=0), n_traj=T, **var); c.run(100)
+    assert not np.allclose(c.get_coords(), xg, atol=1e-3)
+    with pytest.raises(m.SopError) as ei:
+        m.Sop(w.xyz, w.bonds, w.native, p, mode=3)
+    assert ei.value.code == -1

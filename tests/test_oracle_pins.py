@@ -591,3 +591,97 @@ def test_p11_observables_closed_forms():
     # and it is minus the total force the tip exerts on the beads, projected on the tip direction
     _, fb = o.eval_frozen(x0, step=s0)
     assert ft == pytest.approx(float(fb.sum(axis=0) @ np.array([0.0, 0.0, -1.0])), rel=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------- P12 (NEXT-2)
+def _taus_component_matrix(k):
+    """32x32 GF(2) matrix of Tausworthe component k, column j = image of bit j, built from the oracle's own step
+    (valid because the step is linear over GF(2), which the test checks first)."""
+    cols = []
+    for j in range(32):
+        y = np.zeros(4, np.uint32); y[k] = np.uint32(1 << j)
+        sopo.taus_step(y)
+        cols.append(int(y[k]))
+    return cols
+
+
+def _mat_mul(A, B):
+    """(A o B): apply B, then A; matrices as 32 column images."""
+    def app(M, v):
+        out = 0
+        j = 0
+        while v:
+            if v & 1:
+                out ^= M[j]
+            v >>= 1; j += 1
+        return out
+    return [app(A, B[j]) for j in range(32)]
+
+
+def _mat_pow(M, e):
+    R = [1 << j for j in range(32)]
+    while e:
+        if e & 1:
+            R = _mat_mul(M, R)
+        M = _mat_mul(M, M)
+        e >>= 1
+    return R
+
+
+def test_p12_hybrid_taus_linearity_periods_lcg_and_moments():
+    """Alg. 6 with the constants of reading R12.  Pins that do not retype the recurrence:
+    (i) every Tausworthe component is linear over GF(2); (ii) on the k significant bits its transition matrix has
+    order exactly 2^k - 1 for k = 31, 29, 28 (L'Ecuyer's maximal-period condition: any wrong shift or mask breaks it),
+    which gives the period ~2^88 of the three components and, with the 2^32 LCG, the paper's ~2^121 (PAPER.md:177);
+    (iii) the LCG obeys its closed form; (iv) uniform and Box-Muller moments of the output."""
+    r = np.random.default_rng(7)
+    for k in range(3):
+        for _ in range(50):
+            a, b = (int(v) for v in r.integers(0, 2 ** 32, 2, dtype=np.uint64))
+            ya = np.zeros(4, np.uint32); ya[k] = a; sopo.taus_step(ya)
+            yb = np.zeros(4, np.uint32); yb[k] = b; sopo.taus_step(yb)
+            yc = np.zeros(4, np.uint32); yc[k] = a ^ b; sopo.taus_step(yc)
+            assert int(yc[k]) == int(ya[k]) ^ int(yb[k])
+    ident = [1 << j for j in range(32)]
+    for k, bits, factors in ((0, 31, [2147483647]), (1, 29, [233, 1103, 2089]), (2, 28, [3, 5, 29, 43, 113, 127])):
+        M = _taus_component_matrix(k)
+        low = 32 - bits                                   # the low (32 - k) bits of the state are ignored by the recurrence
+        assert all(M[j] == 0 for j in range(low))
+        P = (1 << bits) - 1
+        prod = 1
+        for f in factors:
+            prod *= f
+        assert prod == P
+        hi = lambda Mx: [Mx[j] >> low for j in range(low, 32)]
+        assert hi(_mat_pow(M, P)) == hi(ident)            # M^(2^k - 1) = I on the significant bits ...
+        for f in factors:
+            if P // f > 1:
+                assert hi(_mat_pow(M, P // f)) != hi(ident)   # ... and no proper divisor: the order is exactly 2^k - 1
+    # LCG: y_n = a^n y_0 + c (a^n - 1)/(a - 1) mod 2^32, checked by iterating the oracle against modular arithmetic
+    a, c, y0, n = 1664525, 1013904223, 123456789, 1000
+    y = np.array([2, 8, 16, y0], np.uint32)
+    for _ in range(n):
+        sopo.taus_step(y)
+    geo = 0
+    an = 1
+    for _ in range(n):
+        geo = (geo * a + 1) % 2 ** 32
+        an = (an * a) % 2 ** 32
+    assert int(y[3]) == (an * y0 + c * geo) % 2 ** 32
+    # output statistics: uniform moments of 2^18 draws, and the normals used by a run
+    y = sopo.taus_seed(0xC0FFEE, 11, 3)
+    assert y[0] >= 2 and y[1] >= 8 and y[2] >= 16
+    u = np.array([sopo.taus_step(y) for _ in range(1 << 18)], np.float64) / 2.0 ** 32
+    m = len(u)
+    assert abs(u.mean() - 0.5) < 5 / math.sqrt(12 * m)
+    assert abs(u.var() - 1 / 12) < 5 * math.sqrt(1 / 180 / m)
+    assert abs(np.corrcoef(u[:-1], u[1:])[0, 1]) < 5 / math.sqrt(m)
+    w = gen.free_beads(4000)
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, dict(w.params, rng=1))
+    x0 = o.get_coords().copy()
+    nst = 25
+    o.run(nst)
+    d = o.get_coords() - x0
+    var = 2 * float(np.float32(0.6)) * float(np.float32(2e-3)) * nst
+    assert abs(d.mean()) < 5 * math.sqrt(var / d.size)
+    assert d.var() == pytest.approx(var, rel=5 * math.sqrt(2.0 / d.size))
