@@ -346,6 +346,13 @@ def main():
             "bytes_per_bead_step": main_res["bytes"]["B_fi"], "traffic": traffic, "traffic_source": traffic_src,
             "algorithmic_bytes_per_launch": alg_per_launch,
             "note": "algorithmic bytes / CUDA-event time of the step kernel; the working set is L2/SM resident, so dram traffic is far below the algorithmic bytes (profiles/)"}
+    pr = main_res["profile"]
+    line["list_kernels"] = {
+        "l1_rebuild_us": pr["l1_ms"] * 1e3 / pr["l1_spans"] if pr["l1_spans"] else None, "l1_rebuilds": pr["l1_spans"],
+        "standalone_filter_us": pr["filter_ms"] * 1e3 / pr["filter_spans"] if pr["filter_spans"] else None,
+        "standalone_filters": pr["filter_spans"],
+        "note": "CUDA-event spans inside the library: a1+a2 (+ slot localisation in mode 3) per pair-list rebuild; a3 as its own "
+                "kernel (modes 2/3 filter inside the step kernel, so only the end-of-run / set_coords filters show up here)"}
     line["whole_step_gbs"] = main_res["bytes"]["B_step"] * w.n_beads * T * world / (main_res["us_per_langevin_step"] * 1e-6) / 1e9
 
     if rank == 0 and world == 1:
