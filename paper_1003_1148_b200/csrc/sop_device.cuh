@@ -210,19 +210,26 @@ __device__ __forceinline__ float3 internal_force(const SysDev &S, const float4 *
   return make_float3(fx, fy, fz);
 }
 
-// a7: external forces on one bead (readings R7, R8).
-__device__ __forceinline__ void external_force(const SysDev &S, int i, const float4 &ri, uint32_t tag,
-                                               unsigned long long step, float &fx, float &fy, float &fz, int &flag) {
+// what a7 needs of the step number: spring-base advance and tip centre (computed once per step, off the critical path)
+struct ExtStep { float vs_pull, cx, cy, cz; };
+__device__ __forceinline__ ExtStep ext_step(const SysDev &S, unsigned long long step) {
+  ExtStep e;
+  e.vs_pull = (float)((double)S.pull_v * (double)step);
+  const float vs = (float)((double)S.tip_v * (double)step);
+  e.cx = S.tip_cx + vs * S.tip_nx; e.cy = S.tip_cy + vs * S.tip_ny; e.cz = S.tip_cz + vs * S.tip_nz;
+  return e;
+}
+
+// a7: external forces on one bead (readings R7, R8), the step-dependent scalars given.
+__device__ __forceinline__ void external_force_at(const SysDev &S, int i, const float4 &ri, uint32_t tag, const ExtStep &e,
+                                                  float &fx, float &fy, float &fz, int &flag) {
   if (S.has_pull && (tag & TAG_PULLED)) {
-    float vs = (float)((double)S.pull_v * (double)step);
     float proj = ri.x * S.pull_nx + ri.y * S.pull_ny + ri.z * S.pull_nz - __ldg(&S.pull_adotn[i]);
-    float f = S.pull_k * (vs - proj);
+    float f = S.pull_k * (e.vs_pull - proj);
     fx += f * S.pull_nx; fy += f * S.pull_ny; fz += f * S.pull_nz;
   }
   if (S.tip_on) {
-    float vs = (float)((double)S.tip_v * (double)step);
-    float dx = ri.x - (S.tip_cx + vs * S.tip_nx), dy = ri.y - (S.tip_cy + vs * S.tip_ny),
-          dz = ri.z - (S.tip_cz + vs * S.tip_nz);
+    float dx = ri.x - e.cx, dy = ri.y - e.cy, dz = ri.z - e.cz;
     float g2 = dx * dx + dy * dy + dz * dz;
     float inv_g = rsqrtf(g2);
     float gap = g2 * inv_g - S.tip_R;
@@ -232,6 +239,12 @@ __device__ __forceinline__ void external_force(const SysDev &S, int i, const flo
     float s = 6.0f * S.tip_eps * S.tip_sigma6 * ig2 * ig2 * ig2 * ig * inv_g;
     fx += s * dx; fy += s * dy; fz += s * dz;
   }
+}
+
+// a7: external forces on one bead (readings R7, R8).
+__device__ __forceinline__ void external_force(const SysDev &S, int i, const float4 &ri, uint32_t tag,
+                                               unsigned long long step, float &fx, float &fy, float &fz, int &flag) {
+  external_force_at(S, i, ri, tag, ext_step(S, step), fx, fy, fz, flag);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -595,6 +595,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     float4 *gc = sg + (size_t)(k & 1) * R.chunk, *gnx = sg + (size_t)((k & 1) ^ 1) * R.chunk;
     uint4 *const xc = (k & 1) ? xl1 : xl0, *const xn = (k & 1) ? xl0 : xl1;
     const uint32_t st_c = stamp0 + (uint32_t)k, st_n = st_c + 1u;
+    const ExtStep ext = ext_step(S, step);          // fp64 conversions of the step number: before the waits, not after
     // (b) active halo of layer k: poll until the neighbours have published it
     if (multi && !have_full) {
       const int na = misc[0];
@@ -675,7 +676,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
       float4 out = ri;
       if (!(tag & TAG_FIXED)) {
         float fx = a.x, fy = a.y, fz = a.z;
-        external_force(S, b0 + i, ri, tag, step, fx, fy, fz, flag);
+        external_force_at(S, b0 + i, ri, tag, ext, fx, fy, fz, flag);
         float3 gn;
         if (G > 1) { const float4 g4 = gc[i]; gn = make_float3(g4.x, g4.y, g4.z); }
         else gn = gaussian3(S, tag & TAG_ID_MASK, traj, step);      // thread per bead already: nobody idles
