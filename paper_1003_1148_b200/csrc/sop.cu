@@ -233,6 +233,7 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
     R.off_misc = take(64);
     R.smem_bytes = (int)o;
   };
+  if (getenv("SOP_TEST_NO_PL_SMEM") && !pl.static_l1) pl_want = 0;      // test hook: exercise the L1-rows-in-global path
   // implicit L1: the same region holds the in-kernel cell grid (2 x (cells + 1) ints + 2 x chunk shorts)
   if (pl.static_l1) pl_want = (2 * (RES_GRID_CELLS + 1) * 4 + 4 * chunk + 64) / 2;
   // what is read every step goes to shared memory first (natives), then the L1 rows (read every nb_interval steps)

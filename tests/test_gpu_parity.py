@@ -532,3 +532,20 @@ def test_hybrid_taus_noise_matches_the_oracle(var):
     with pytest.raises(m.SopError) as ei:
         m.Sop(w.xyz, w.bonds, w.native, p, mode=3)
     assert ei.value.code == -1
+
+
+def test_mode3_l1_rows_read_from_global_memory_when_they_do_not_fit():
+    """The filter normally walks L1 rows that were copied to shared memory; a chunk whose rows do not fit reads them
+    from global memory instead.  SOP_TEST_NO_PL_SMEM forces that path: identical results, bit for bit."""
+    w = gen.two_chains(150, 3, R_pl=20.0)
+    a = sop().from_workload(w, mode=3, chunk_beads=60); a.run(230)
+    os.environ["SOP_TEST_NO_PL_SMEM"] = "1"
+    try:
+        b = sop().from_workload(w, mode=3, chunk_beads=60); b.run(230)
+    finally:
+        del os.environ["SOP_TEST_NO_PL_SMEM"]
+    assert np.array_equal(a.get_coords(), b.get_coords())
+    ca, ia, _ = a.get_lists(2); cb, ib, _ = b.get_lists(2)
+    assert rows_equal(ca, ia, cb, ib)
+    o = sopo.from_workload(w); o.run(230)
+    assert np.abs(b.get_coords() - o.get_coords()).max() <= 3e-3
