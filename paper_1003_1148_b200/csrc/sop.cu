@@ -237,13 +237,14 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
   // implicit L1: the same region holds the in-kernel cell grid (2 x (cells + 1) ints + 2 x chunk shorts)
   if (pl.static_l1) pl_want = (2 * (RES_GRID_CELLS + 1) * 4 + 4 * chunk + 64) / 2;
   // what is read every step goes to shared memory first (natives), then the L1 rows (read every nb_interval steps)
-  carve(true, pl_want);
+  const bool nat_ok = getenv("SOP_TEST_NO_NAT_SMEM") == nullptr;          // test hook: natives stay in global memory
+  carve(nat_ok, pl_want);
   if (o > 232448 && pl.static_l1) carve(false, pl_want);
   if (o > 232448 && !pl.static_l1) {
     // the L1 rows get what is left (the kernel reads them from global memory if a chunk's rows do not fit at run time)
-    carve(true, 0);
+    carve(nat_ok, 0);
     const long long left = (232448 - (long long)o) / 2 - 16;
-    if (left > 4 * chunk) carve(true, (int)std::min<long long>(pl_want, left));
+    if (left > 4 * chunk) carve(nat_ok, (int)std::min<long long>(pl_want, left));
   }
   if (o > 232448 && !pl.static_l1) carve(false, 0);
   if (o > 232448) { pl.res_why = "chunk state does not fit the 227 KB of shared memory of an SM"; return; }

@@ -549,3 +549,19 @@ def test_mode3_l1_rows_read_from_global_memory_when_they_do_not_fit():
     assert rows_equal(ca, ia, cb, ib)
     o = sopo.from_workload(w); o.run(230)
     assert np.abs(b.get_coords() - o.get_coords()).max() <= 3e-3
+
+
+@pytest.mark.parametrize("var", [dict(chunk_beads=60, lanes_per_bead=4), dict(lanes_per_bead=1), dict(lanes_per_bead=2)], ids=str)
+def test_mode3_native_table_in_global_memory(var):
+    """Chunks whose native table does not fit shared memory read it from global memory (packed per chunk, or transposed
+    for a one-chunk trajectory with one lane per bead).  SOP_TEST_NO_NAT_SMEM forces those paths: same results."""
+    w = gen.two_chains(150, 3, R_pl=20.0)
+    a = sop().from_workload(w, mode=3, **var); a.run(130)
+    os.environ["SOP_TEST_NO_NAT_SMEM"] = "1"
+    try:
+        b = sop().from_workload(w, mode=3, **var); b.run(130)
+    finally:
+        del os.environ["SOP_TEST_NO_NAT_SMEM"]
+    assert np.array_equal(a.get_coords(), b.get_coords())
+    o = sopo.from_workload(w); o.run(130)
+    assert np.abs(b.get_coords() - o.get_coords()).max() <= 2e-3
