@@ -322,20 +322,26 @@ __device__ __forceinline__ void filter_row_warp(const SysDev &S, const float4 *_
   int *dst = S.nb_idx + (size_t)g * S.cap_nb;
   const float4 ri = ldpos<NC>(pos_t + i);
   int n = 0;
-  for (int base = 0; base < cnt1; base += 32) {
-    int p = base + lane;
-    int j = -1;
-    bool pass = false;
-    if (p < cnt1) {
-      j = src[p];
-      pass = pred32(ri, ldpos<NC>(pos_t + j), S.R_nb2);
+  // 128 candidates per iteration: four index loads, then four coordinate gathers in flight per lane (the gathers are
+  // L2 round trips for large systems), then four ordered compactions
+  for (int base = 0; base < cnt1; base += 128) {
+    int j[4];
+    float4 rj[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int p = base + 32 * u + lane; j[u] = p < cnt1 ? src[p] : -1; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) rj[u] = j[u] >= 0 ? ldpos<NC>(pos_t + j[u]) : ri;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (base + 32 * u >= cnt1) break;
+      const bool pass = j[u] >= 0 && pred32(ri, rj[u], S.R_nb2);
+      unsigned m = __ballot_sync(0xffffffffu, pass);
+      if (pass) {
+        int slot = n + __popc(m & ((1u << lane) - 1u));
+        if (slot < S.cap_nb) dst[slot] = j[u];
+      }
+      n += __popc(m);
     }
-    unsigned m = __ballot_sync(0xffffffffu, pass);
-    if (pass) {
-      int slot = n + __popc(m & ((1u << lane) - 1u));
-      if (slot < S.cap_nb) dst[slot] = j;
-    }
-    n += __popc(m);
   }
   if (n > S.cap_nb) { flag |= FLAG_NB_OVERFLOW; n = S.cap_nb; }
   if (lane == 0) S.nb_cnt[g] = n;
