@@ -352,9 +352,13 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   __syncthreads();
 #ifdef SOP_PHASE_CLOCKS
   long long pc_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, pc_t = clock64();
-#define SOP_TICK(n) { const long long now_ = clock64(); pc_acc[n] += now_ - pc_t; pc_t = now_; }
+  int pc_dep = 0;
+// the clock reads and the block barriers are tied by register dependences, or ptxas moves the reads across the barriers
+#define SOP_TICK(n) { long long now_; asm volatile("mov.u64 %0, %%clock64;" : "=l"(now_) : "r"(pc_dep) : "memory"); pc_acc[n] += now_ - pc_t; pc_t = now_; }
+#define SOP_SYNC() { pc_dep = __syncthreads_or((int)(pc_t >> 63)); }
 #else
 #define SOP_TICK(n)
+#define SOP_SYNC() __syncthreads()
 #endif
   // a3: Alg. 3 on the own rows, candidates and coordinates from shared memory
   auto filter_rows = [&](const float4 *P) {
@@ -457,7 +461,6 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         }
       }
       __syncthreads();
-      SOP_TICK(5)                                                                          // in-kernel cell grid
       // one thread per row: with a whole trajectory in the chunk there are about as many rows as threads, and a
       // private counter compacts without ballots (12x fewer warp instructions than a warp per row, measured)
       for (int il = tid; il < n_own; il += bd) {
@@ -609,8 +612,8 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     }
     have_full = false;
     SOP_TICK(0)                                                                            // halo poll
-    __syncthreads();
-    SOP_TICK(1)                                                                            // waiting for the CTA
+    SOP_SYNC();
+    SOP_TICK(1)                                                                            // waiting for the slowest poller
     // (d1) a4..a6: internal force, G lanes per bead (Alg. 2; no distance test in the loop, R3c)
     for (int base = 0; base < n_own; base += groups) {
       const bool valid = base + grp < n_own;
@@ -667,7 +670,8 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
       if (valid && lane == 0) sforce[il] = make_float4(fx, fy, fz, 0.f);
     }
     SOP_TICK(2)                                                                            // pair forces
-    __syncthreads();
+    SOP_SYNC();
+    SOP_TICK(3)                                                                            // waiting for the slowest warp
     // (d2) a7 + a9: thread per bead; the other end of the block draws the next step's noise (a8)
     for (int i = tid; i < n_own; i += bd) {
       const float4 ri = pc[i];
@@ -694,7 +698,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         }
       }
     }
-    SOP_TICK(3)                                                                            // update + noise
+    SOP_TICK(4)                                                                            // update + noise
     // (e) a3: Alg. 3 on the own rows from the coordinates just written (list invariant)
     if (--until_filter == 0) {
       until_filter = nb_interval;
@@ -706,15 +710,12 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
             while (!xch_try(src, st_n, v)) {}
             pn[n_own + q] = v;
           }
-        SOP_TICK(4)                                                                        // whole-halo poll
         __syncthreads();
-        SOP_TICK(5)
         filter_rows(pn);
-        SOP_TICK(6)                                                                        // Alg. 3 rows
         after_filter();
         have_full = true;
       }
-      SOP_TICK(7)                                                                          // active set, offsets
+      SOP_TICK(5)                                                                          // filter (whole-halo poll, rows, active set)
     }
   }
 #ifdef SOP_PHASE_CLOCKS
