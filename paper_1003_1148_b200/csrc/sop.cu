@@ -231,6 +231,8 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
     R.off_bm = take((size_t)(halo_cap / 32 + 1) * 4);
     R.off_sbm = take((size_t)(halo_cap / 32 + 1) * 4);
     R.off_misc = take(64);
+    R.off_order = take((size_t)chunk * 2);
+    R.off_hist = take(64 * 4);
     R.smem_bytes = (int)o;
   };
   if (getenv("SOP_TEST_NO_PL_SMEM") && !pl.static_l1) pl_want = 0;      // test hook: exercise the L1-rows-in-global path

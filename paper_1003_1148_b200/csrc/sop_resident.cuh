@@ -38,7 +38,7 @@ struct ResDev {
   uint4 *xch;                 // [2][T*N][2]  {x, stamp, y, stamp, z, stamp, -, -}: one 32-byte slot per bead
   // shared-memory carve-up (bytes from the start of dynamic shared memory), computed by the host
   int off_pos, off_g, off_carry, off_tag, off_force, off_nb, off_cnt, off_plcnt, off_plofs, off_pl, off_natq,
-      off_nat, off_bond, off_active, off_bm, off_sbm, off_misc;
+      off_nat, off_bond, off_active, off_bm, off_sbm, off_misc, off_order, off_hist;
   int nb_si;                  // L2 row i starts at nb[i * nb_si] (an odd number of 32-bit words: conflict-free)
   int nat_smem;               // the chunk's native table is copied to shared memory (its nat_cap entries fit)
   int nat_cap;                // largest number of native entries of a chunk
@@ -243,6 +243,8 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   int2 *sbond = (int2 *)(smem_raw + R.off_bond);                     // [chunk][cap_b]
   unsigned short *active = (unsigned short *)(smem_raw + R.off_active);
   uint32_t *bm = (uint32_t *)(smem_raw + R.off_bm), *sbm = (uint32_t *)(smem_raw + R.off_sbm);
+  unsigned short *order = (unsigned short *)(smem_raw + R.off_order);     // own beads by descending native degree
+  int *hist = (int *)(smem_raw + R.off_hist);                              // [64] scratch of that counting sort
   int *misc = (int *)(smem_raw + R.off_misc);                        // [0] active halo slots, [2..7] bounding box of the in-kernel grid
 
   const int tc = blockIdx.x, t = tc / R.C, c = tc - t * R.C;
@@ -326,7 +328,17 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     }
   }
   for (int w = tid; w < HW; w += bd) sbm[w] = 0u;
+  for (int b = tid; b < 64; b += bd) hist[b] = 0;
   __syncthreads();
+  // processing order of the pair phase: own beads by descending native degree (counting sort), so that the groups of a
+  // warp run the same number of native iterations and fewer warp-level gathers carry idle lanes.  Which group handles
+  // a bead does not change its force (lane = position in the list mod G), so ties may fall either way.
+  for (int i = tid; i < n_own; i += bd) atomicAdd(&hist[63 - min(63, natq[i + 1] - natq[i])], 1);
+  __syncthreads();
+  if (tid == 0) { int run = 0; for (int b = 0; b < 64; ++b) { const int c2 = hist[b]; hist[b] = run; run += c2; } }
+  __syncthreads();
+  for (int i = tid; i < n_own; i += bd)           // one lane per bead: keep thread i on bead i (coalesced table reads)
+    order[G > 1 ? atomicAdd(&hist[63 - min(63, natq[i + 1] - natq[i])], 1) : i] = (unsigned short)i;
   scan_counts(plcnt_s, plofs, true);
   __syncthreads();
   const bool pl_in_smem = !R.implicit_l1 && R.pl_cap > 0 && plofs[n_own] <= R.pl_cap;
@@ -617,7 +629,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     // (d1) a4..a6: internal force, G lanes per bead (Alg. 2; no distance test in the loop, R3c)
     for (int base = 0; base < n_own; base += groups) {
       const bool valid = base + grp < n_own;
-      const int il = valid ? base + grp : n_own - 1;
+      const int il = order[valid ? base + grp : n_own - 1];
       const float4 ri = pc[il];
       float fx = 0.f, fy = 0.f, fz = 0.f;
       if (valid) {
