@@ -520,7 +520,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
       const int frow = tid / LPR, flane = tid & (LPR - 1), fgroups = bd / LPR;
       for (int base = 0; base < n_own; base += fgroups) {
         const bool valid = base + frow < n_own;
-        const int il = valid ? base + frow : n_own - 1;
+        const int il = order[valid ? base + frow : n_own - 1];      // dense beads together: similar L1 row lengths per warp
         const int cnt1 = valid ? (int)plcnt_s[il] : 0;
         const int nw = (cnt1 + 1) >> 1;
         const float4 ri = P[il];
