@@ -650,11 +650,12 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         }
         // a5: native contacts   V = eps [(r0/r)^12 - 2 (r0/r)^6]   (per-contact eps only when the topology has it)
         const int q1 = natq[il + 1];
-        auto natives = [&](auto has_eps_t) {
-          constexpr bool HAS_EPS = decltype(has_eps_t)::value;
+        auto natives = [&](auto has_eps_t, auto in_smem_t) {
+          constexpr bool HAS_EPS = decltype(has_eps_t)::value, IN_SMEM = decltype(in_smem_t)::value;
           const int q0 = natq[il];
           for (int q = q0 + lane; q < q1; q += G) {
-            const int2 en = R.nat_T ? __ldg(&R.nat_T[(size_t)(q - q0) * R.nat_tpad + il]) : natp[q];
+            const int2 en = IN_SMEM ? snat[q - qbase]           // a plain LDS.64 (the generic pointer costs address checks)
+                                    : R.nat_T ? __ldg(&R.nat_T[(size_t)(q - q0) * R.nat_tpad + il]) : natp[q];
             float e12 = K.eps12;
             if (HAS_EPS) e12 = 12.0f * __ldg(&nat_eps[q]);
             const float4 rj = pc[en.x];
@@ -663,7 +664,9 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
             fx += s * dx; fy += s * dy; fz += s * dz;
           }
         };
-        if (nat_eps) natives(std::true_type{}); else natives(std::false_type{});
+        if (nat_eps) natives(std::true_type{}, std::false_type{});
+        else if (R.nat_smem) natives(std::false_type{}, std::true_type{});
+        else natives(std::false_type{}, std::false_type{});
         // a6: non-native repulsion   V = eps_r (sigma/r)^6; two slots per 32-bit word, odd rows end in the dummy slot
         const uint32_t *row32 = (const uint32_t *)(nb + (size_t)il * R.nb_si);
         const int n2 = ((int)cnt_s[il] + 1) >> 1;
