@@ -518,14 +518,17 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
       int LPR = 1;
       while (LPR < 32 && 2 * LPR * n_own <= bd) LPR <<= 1;
       const int frow = tid / LPR, flane = tid & (LPR - 1), fgroups = bd / LPR;
+      auto rows_loop = [&](auto in_smem_t) {
+      constexpr bool IN_SMEM = decltype(in_smem_t)::value;     // plain LDS when the rows are resident, else global loads
       for (int base = 0; base < n_own; base += fgroups) {
         const bool valid = base + frow < n_own;
         const int il = order[valid ? base + frow : n_own - 1];      // dense beads together: similar L1 row lengths per warp
         const int cnt1 = valid ? (int)plcnt_s[il] : 0;
         const int nw = (cnt1 + 1) >> 1;
         const float4 ri = P[il];
-        const uint32_t *src = pl_in_smem ? (const uint32_t *)(spl + plofs[il])
-                                         : (const uint32_t *)(R.pl_loc + (inst0 + b0 + il) * S.cap_pl);
+        const uint32_t *gsrc = (const uint32_t *)(R.pl_loc + (inst0 + b0 + il) * S.cap_pl);
+        const uint32_t *ssrc = (const uint32_t *)(spl + (IN_SMEM ? plofs[il] : 0));
+        auto word = [&](int w) -> uint32_t { return IN_SMEM ? ssrc[w] : __ldg(gsrc + w); };
         unsigned short *row = nb + (size_t)il * R.nb_si;
         const int rounds = __reduce_max_sync(0xffffffffu, (nw + 32 * LPR - 1) / (32 * LPR));
         int n = 0;
@@ -537,7 +540,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
           const int wend = min(per, rwn - flane * per);
 #pragma unroll 4
           for (int k2 = 0; k2 < wend; ++k2) {
-            const uint32_t u = src[w0 + k2];
+            const uint32_t u = word(w0 + k2);
             const bool pa = pred32(ri, P[u & 0xFFFFu], S.R_nb2);
             const bool pb = 2 * (w0 + k2) + 1 < cnt1 && pred32(ri, P[u >> 16], S.R_nb2);
             mask |= (unsigned long long)(pa ? 1u : 0u) << (2 * k2);
@@ -551,7 +554,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
           while (mask) {
             const int bit = __ffsll((long long)mask) - 1;
             mask &= mask - 1;
-            const uint32_t u = src[w0 + (bit >> 1)];
+            const uint32_t u = word(w0 + (bit >> 1));
             if (at < cap_nb) row[at] = (unsigned short)((bit & 1) ? (u >> 16) : (u & 0xFFFFu));
             ++at;
           }
@@ -560,6 +563,8 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         if (n > cap_nb) { flag |= FLAG_NB_OVERFLOW; n = cap_nb; }
         if (valid && flane == 0) { cnt_s[il] = (unsigned short)n; if (n & 1) row[n] = DUMMY; }
       }
+      };
+      if (pl_in_smem) rows_loop(std::true_type{}); else rows_loop(std::false_type{});
     }
   };
   // active halo = static part + halo slots of the current L2 rows
