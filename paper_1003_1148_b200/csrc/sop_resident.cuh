@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         const int j = row[p];
         dst[p] = (unsigned short)((j >= b0 && j < b1) ? j - b0 : n_own + lower_bound_dev(hgid, n_halo, j));
       }
-      if (wlane == 0) { cnt_s[il] = (unsigned short)cnt; if (cnt & 1) dst[cnt] = DUMMY; }
+      if (wlane == 0) { cnt_s[il] = (unsigned short)cnt; for (int k4 = cnt; k4 & 3; ++k4) dst[k4] = DUMMY; }
     }
   }
   for (int w = tid; w < HW; w += bd) sbm[w] = 0u;
@@ -390,7 +390,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
           n += __popc(m);
         }
         if (n > cap_nb) { flag |= FLAG_NB_OVERFLOW; n = cap_nb; }
-        if (wlane == 0) { cnt_s[il] = (unsigned short)n; if (n & 1) row[n] = DUMMY; }
+        if (wlane == 0) { cnt_s[il] = (unsigned short)n; for (int k4 = n; k4 & 3; ++k4) row[k4] = DUMMY; }
       }
     } else if (R.implicit_l1) {
       // static all-pairs L1 (one chunk = the whole trajectory): L2 row of i = every j != i within R_nb that is not
@@ -509,7 +509,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         }
         if (n > cap_nb) { flag |= FLAG_NB_OVERFLOW; n = cap_nb; }
         cnt_s[il] = (unsigned short)n;
-        if (n & 1) row[n] = DUMMY;
+        for (int k4 = n; k4 & 3; ++k4) row[k4] = DUMMY;
       }
     } else {
       // LPR lanes per row (as many as the block has per own bead, a power of two): a lane tests a contiguous run of
@@ -561,7 +561,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
           n += total;
         }
         if (n > cap_nb) { flag |= FLAG_NB_OVERFLOW; n = cap_nb; }
-        if (valid && flane == 0) { cnt_s[il] = (unsigned short)n; if (n & 1) row[n] = DUMMY; }
+        if (valid && flane == 0) { cnt_s[il] = (unsigned short)n; for (int k4 = n; k4 & 3; ++k4) row[k4] = DUMMY; }
       }
       };
       if (pl_in_smem) rows_loop(std::true_type{}); else rows_loop(std::false_type{});
@@ -672,18 +672,25 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         if (nat_eps) natives(std::true_type{}, std::false_type{});
         else if (R.nat_smem) natives(std::false_type{}, std::true_type{});
         else natives(std::false_type{}, std::false_type{});
-        // a6: non-native repulsion   V = eps_r (sigma/r)^6; two slots per 32-bit word, odd rows end in the dummy slot
-        const uint32_t *row32 = (const uint32_t *)(nb + (size_t)il * R.nb_si);
-        const int n2 = ((int)cnt_s[il] + 1) >> 1;
-        for (int p = lane; p < n2; p += G) {
-          const uint32_t u = row32[p];
-          const float4 ra = pc[u & 0xFFFFu], rb = pc[u >> 16];
+        // a6: non-native repulsion   V = eps_r (sigma/r)^6; four slots per 8-byte word (rows are padded to a multiple
+        // of four with the dummy slot): one index load, four gathers in flight
+        const uint2 *row64 = (const uint2 *)(nb + (size_t)il * R.nb_si);
+        const int n4 = ((int)cnt_s[il] + 3) >> 2;
+        for (int p = lane; p < n4; p += G) {
+          const uint2 w = row64[p];
+          const float4 ra = pc[w.x & 0xFFFFu], rb = pc[w.x >> 16], rc = pc[w.y & 0xFFFFu], rd = pc[w.y >> 16];
           const float ax = ri.x - ra.x, ay = ri.y - ra.y, az = ri.z - ra.z;
           const float bx = ri.x - rb.x, by = ri.y - rb.y, bz = ri.z - rb.z;
+          const float cx = ri.x - rc.x, cy = ri.y - rc.y, cz = ri.z - rc.z;
+          const float dx = ri.x - rd.x, dy = ri.y - rd.y, dz = ri.z - rd.z;
           const float sa = rep_s3(ax * ax + ay * ay + az * az, K.c_rep_f);
           const float sb = rep_s3(bx * bx + by * by + bz * bz, K.c_rep_f);
+          const float sc = rep_s3(cx * cx + cy * cy + cz * cz, K.c_rep_f);
+          const float sd = rep_s3(dx * dx + dy * dy + dz * dz, K.c_rep_f);
           fx += sa * ax; fy += sa * ay; fz += sa * az;
           fx += sb * bx; fy += sb * by; fz += sb * bz;
+          fx += sc * cx; fy += sc * cy; fz += sc * cz;
+          fx += sd * dx; fy += sd * dy; fz += sd * dz;
         }
       }
       if (G > 1) { fx = group_sum<G>(fx); fy = group_sum<G>(fy); fz = group_sum<G>(fz); }
