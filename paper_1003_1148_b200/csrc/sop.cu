@@ -14,6 +14,7 @@
 #include "sop_kernels.cuh"
 #include "sop_persistent.cuh"
 #include "sop_resident.cuh"
+#include "sop_resident2.cuh"
 
 using namespace sop;
 
@@ -39,7 +40,12 @@ struct Plan {                     // everything that depends only on (topology, 
   std::string res_why;
   int res_lanes = 1, res_block = 1024, res_nat_rows = 0;
   ResDev R;
-  size_t off_nhalo, off_hgid, off_plloc, off_natloc, off_bondloc, off_xch;
+  size_t off_nhalo, off_hgid, off_plloc, off_natloc, off_bondloc, off_xch, off_xchf;
+  // mode 3, several chunks per trajectory: the second resident kernel (sop_resident2.cuh) when its plan fits
+  bool res2_ok = false;
+  int res2_block = 0;
+  Res2Dev R2;
+  size_t off_plarr, off_plg;
 };
 
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -69,7 +75,9 @@ struct sop_handle {
   int coop_block_size = 0;
   int num_sms = 0;
   unsigned *S_bar = nullptr;      // grid-barrier counter of the persistent kernel
-  ResDev R;                       // mode 3
+ ResDev R;                       // mode 3
+  Res2Dev R2;
+  const void *res2_fn = nullptr;
   int obs_a = 0, obs_b = 0;       // internal indices of the two ends of the end-to-end distance
   const void *res_fn = nullptr;
   uint32_t res_launch_id = 0;
@@ -150,6 +158,93 @@ uint32_t part1by2(uint32_t v) {   // spread the low 10 bits of v
   v = (v | (v << 4)) & 0x030C30C3;
   v = (v | (v << 2)) & 0x09249249;
   return v;
+}
+
+// ---- mode 3, several chunks: plan of the second resident kernel (sop_resident2.cuh).  Called at the end of plan_resident
+// (chunking and halo capacity are shared).  Leaves res2_ok = false when the chunk state does not fit; the first kernel
+// then runs the multi-chunk case too.
+void plan_resident2(const sop_topology *tp, const sop_params *p, const std::vector<double> &x, Plan &pl) {
+  const ResDev &R = pl.R;
+  Res2Dev &Q = pl.R2;
+  memset(&Q, 0, sizeof(Q));
+  pl.res2_ok = false;
+  if (R.C <= 1 || pl.static_l1 || getenv("SOP_TEST_OLD_RESIDENT")) return;
+  const int N = pl.N, chunk = R.chunk;
+  const int max_groups = (32 - R2_SERVICE_WARPS) * 4;
+  const int P = (chunk + max_groups - 1) / max_groups;
+  if (P > R2_MAXP) return;
+  if ((p->lanes_per_bead != 0 && p->lanes_per_bead != 8) || p->block_size > 0) return;   // explicit launch shapes: first design
+  Q.P = P;
+  Q.n_cwarps = (chunk + 4 * P - 1) / (4 * P);
+  pl.res2_block = 32 * (Q.n_cwarps + R2_SERVICE_WARPS);
+  if (chunk > pl.res2_block || R.halo_cap > 32760 || pl.cap_pl > 496 || pl.cap_nb > 240 || pl.cap_b > 8) return;   // (15-bit partner codes, 64-bit survivor masks)
+  Q.own_pad = (chunk + 7) / 8 * 8; Q.halo_pad = (R.halo_cap + 7) / 8 * 8;
+  Q.own_stride = Q.own_pad + 8; Q.halo_stride = Q.halo_pad + 8;
+  Q.cap_arr = (pl.cap_pl + 7) / 8 * 8 + 16;
+  // force rows of a chunk: natives + partners within 1.05 R_nb of the native structure + the padding of two segments
+  std::vector<long long> per(R.C, 0);
+  {
+    std::vector<int> nnb(N, 0);
+    visit_neighbors(x, N, (double)p->R_nb * 1.05, [&](int i, int) { nnb[i]++; });
+    std::vector<int> nnat(N, 0);
+    for (int c2 = 0; c2 < tp->n_native; ++c2) {          // natives the neighbour count above does not contain
+      const int i = tp->native[2 * c2], j = tp->native[2 * c2 + 1];
+      const double dx = x[3 * i] - x[3 * j], dy = x[3 * i + 1] - x[3 * j + 1], dz = x[3 * i + 2] - x[3 * j + 2];
+      if (dx * dx + dy * dy + dz * dz >= (double)p->R_nb * 1.05 * (double)p->R_nb * 1.05) { nnat[i]++; nnat[j]++; }
+    }
+    for (int i = 0; i < N; ++i) per[pl.iperm[i] / chunk] += nnb[i] + nnat[i] + 8;
+  }
+  long long want = (long long)(*std::max_element(per.begin(), per.end()) * 1.15) + 64;
+  want = std::min<long long>((want + 7) / 8 * 8, 65528LL * 8);
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = (o + bytes + 127) / 128 * 128; return (int)at; };
+  auto carve = [&](long long rows_cap) {
+    o = 0;
+    Q.rows_cap = (int)rows_cap;
+    Q.off_own = take(2 * (size_t)Q.own_stride * 16);
+    Q.off_halo = take(2 * (size_t)Q.halo_stride * 16);
+    Q.off_rows = take((size_t)rows_cap * 8);
+    Q.off_eps = take(tp->native_eps ? (size_t)rows_cap * 4 : 0);
+    Q.off_kbase = take((size_t)chunk * 16);
+    Q.off_ext = take(32);
+    Q.off_g = take(2 * (size_t)chunk * 16);
+    Q.off_carry = take(pl.comp ? (size_t)chunk * 16 : 0);
+    Q.off_tag = take((size_t)chunk * 4);
+    Q.off_rowofs = take(((size_t)chunk + 1) * 2);
+    Q.off_rowg = take((size_t)chunk * 2);
+    Q.off_nat = take((size_t)R.nat_cap * 8);
+    Q.off_natq = take(((size_t)chunk + 1) * 4);
+    Q.off_bond = take((size_t)chunk * pl.cap_b * 8);
+    Q.off_tmp = take((size_t)chunk * pl.cap_nb * 2);
+    Q.off_cnt = take((size_t)chunk * 2);
+    Q.off_active = take((size_t)R.halo_cap * 2);
+    Q.off_bm = take((size_t)(R.halo_cap / 32 + 1) * 4);
+    Q.off_sbm = take((size_t)(R.halo_cap / 32 + 1) * 4);
+    Q.off_misc = take(64);
+    Q.off_order = take((size_t)chunk * 2);
+    Q.off_hist = take((size_t)std::max(64, (pl.res2_block / 32) * 64) * 4);
+    Q.off_taus = take(p->rng == 1 ? (size_t)chunk * 16 : 0);
+    Q.smem_bytes = (int)o;
+  };
+  {
+    const double e12 = 12.0 * (double)p->eps_native;
+    const double a_ref = e12 > 0.0 ? e12 : 1.0;
+    Q.a_ref = (float)a_ref;
+    Q.par_rep = (float)(-std::cbrt(6.0 * (double)p->eps_rep * std::pow((double)p->sigma, 6.0) / (double)Q.a_ref));
+  }
+  const int per_entry = tp->native_eps ? 12 : 8;
+  carve(want);
+  if (o > 232448) {                       // the rows get what is left, if that is still most of what they may need
+    const long long fixed = (long long)o - want * per_entry;
+    const long long left = (232448 - fixed - 512) / per_entry / 8 * 8;
+    if (left * 10 < want * 8) return;
+    carve(left);
+    if (o > 232448) return;
+  }
+  pl.res2_ok = true;
+  if (getenv("SOP_DEBUG_PLAN"))
+    fprintf(stderr, "[sop plan] mode 3 (second kernel): P=%d compute warps=%d block=%d rows_cap=%d cap_arr=%d smem=%d B\n",
+            Q.P, Q.n_cwarps, pl.res2_block, Q.rows_cap, Q.cap_arr, Q.smem_bytes);
 }
 
 // ---- mode 3 plan: chunks, lanes, halo capacity from the native structure, shared-memory carve-up ------------
@@ -259,6 +354,7 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
     R.nat_tpad = (N + 31) / 32 * 32;
   }
   if ((size_t)((N + 31) / 32) * 8 > 200000) { pl.res_why = "n_beads too large for the localise bitmap"; return; }
+  plan_resident2(tp, p, x, pl);
   if (getenv("SOP_DEBUG_PLAN"))
     fprintf(stderr, "[sop plan] mode 3: C=%d chunk=%d lanes=%d block=%d halo_cap=%d cap_nb=%d cap_pl=%d nat_smem=%d pl_cap=%d smem=%d B\n",
             R.C, R.chunk, pl.res_lanes, pl.res_block, R.halo_cap, pl.cap_nb, pl.cap_pl, R.nat_smem, R.pl_cap, R.smem_bytes);
@@ -353,9 +449,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   if (pl.block % 32 || pl.block > 1024) return fail(SOP_E_ARG, "block_size must be a multiple of 32, <= 1024");
   if (p->mode < 0 || p->mode > 3) return fail(SOP_E_ARG, "mode must be 0, 1, 2 or 3");
   if (p->rng != 0 && p->rng != 1) return fail(SOP_E_ARG, "rng must be 0 (Philox) or 1 (Hybrid Taus)");
-  if (p->rng == 1 && p->mode == 3) return fail(SOP_E_ARG, "rng = 1 (Hybrid Taus) runs in modes 1 and 2 only");
   pl.mode = p->mode;
-  if (p->rng == 1 && pl.mode == 0) pl.mode = inst > 100000 ? 1 : 2;
   if (pl.mode == 0 || pl.mode == 3) {
     plan_resident(tp, p, x, pl);
     if (pl.mode == 3 && !pl.res_ok) return fail(SOP_E_ARG, "mode 3 is not possible here: " + pl.res_why);
@@ -401,6 +495,9 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
     pl.off_natloc = take(multi ? (size_t)T * pl.n_nat_entries * 8 : (size_t)pl.res_nat_rows * R.nat_tpad * 8);
     pl.off_bondloc = take(multi ? I * pl.cap_b * 8 : 0);
     pl.off_xch = take(multi ? 2 * I * 32 : 0);
+    pl.off_xchf = take(multi ? 2 * I * 32 : 0);
+    pl.off_plarr = take(pl.res2_ok ? I * pl.R2.cap_arr * 2 : 0);
+    pl.off_plg = take(pl.res2_ok ? I * 2 : 0);
   }
   pl.total = o;
   return SOP_OK;
@@ -496,7 +593,9 @@ int read_flags(sop_handle *h) {
   CUDA_OK(cudaMemcpyAsync(&flags, h->S.flags, 4, cudaMemcpyDeviceToHost, h->stream));
   CUDA_OK(cudaStreamSynchronize(h->stream));
   if (!flags) return SOP_OK;
-  CUDA_OK(cudaMemsetAsync(h->S.flags, 0, 4, h->stream));
+  CUDA_OK(cudaMemsetAsync(h->S.flags, 0, 8, h->stream));          // the flag word and the abort word of the exchange
+  if (flags & FLAG_EXCHANGE_TIMEOUT)
+    return fail(SOP_E_CUDA, "mode 3: a chunk waited too long for a neighbour's coordinates (exchange time-out); the run is invalid", h);
   if (flags & FLAG_NONFINITE) return fail(SOP_E_NONFINITE, "non-finite coordinate or bead inside the indenter", h);
   if (flags & FLAG_FENE) return fail(SOP_E_FENE, "a bond reached |r - r0| >= R0", h);
   if (flags & FLAG_PL_OVERFLOW) return fail(SOP_E_LIST_OVERFLOW, "pair-list row exceeded cap_pl", h);
@@ -566,6 +665,20 @@ const void *resident_kernel(int lanes, bool comp) {
   }
 }
 
+template <bool COMP, bool EPS>
+const void *res2_fn_p(int P) {
+  switch (P) {
+    case 1: return (const void *)k_res2<COMP, EPS, 1>;
+    case 2: return (const void *)k_res2<COMP, EPS, 2>;
+    case 3: return (const void *)k_res2<COMP, EPS, 3>;
+    default: return (const void *)k_res2<COMP, EPS, 4>;
+  }
+}
+const void *res2_kernel(bool comp, bool eps, int P) {
+  if (comp) return eps ? res2_fn_p<true, true>(P) : res2_fn_p<true, false>(P);
+  return eps ? res2_fn_p<false, true>(P) : res2_fn_p<false, false>(P);
+}
+
 int resident_prepare(sop_handle *h) {
   const Plan &pl = h->plan;
   h->R = pl.R;
@@ -573,8 +686,15 @@ int resident_prepare(sop_handle *h) {
   char *w = h->ws;
   R.n_halo = (int *)(w + pl.off_nhalo); R.halo_gid = (int *)(w + pl.off_hgid);
   R.pl_loc = (unsigned short *)(w + pl.off_plloc); R.nat_pack = (int2 *)(w + pl.off_natloc);
-  R.bond_pack = (int2 *)(w + pl.off_bondloc); R.xch = (uint4 *)(w + pl.off_xch);
+  R.bond_pack = (int2 *)(w + pl.off_bondloc); R.xch = (uint4 *)(w + pl.off_xch); R.xchf = (uint4 *)(w + pl.off_xchf);
   R.nat_T = nullptr;
+  R.skew_chunk = 0; R.skew_period = 1; R.skew_ns = 0;
+  if (const char *sk = getenv("SOP_TEST_SKEW")) {        // test hook "chunk,period,ns": one chunk runs late on some steps
+    int a = 0, b = 1, c = 0;
+    if (sscanf(sk, "%d,%d,%d", &a, &b, &c) == 3 && b > 0) { R.skew_chunk = a; R.skew_period = b; R.skew_ns = c; }
+  }
+  h->R2 = pl.R2;
+  h->R2.pl_arr = (unsigned short *)(w + pl.off_plarr); h->R2.pl_g = (uchar2 *)(w + pl.off_plg);
   if (R.nat_tpad > 0) {
     R.nat_T = (int2 *)(w + pl.off_natloc);
     k_transpose_nat<<<(h->S.N + 255) / 256, 256, 0, h->stream>>>(h->S, R);
@@ -586,6 +706,12 @@ int resident_prepare(sop_handle *h) {
   int occ = 0;
   CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->res_fn, pl.res_block, R.smem_bytes));
   if (occ < 1) return fail(SOP_E_CUDA, "resident kernel does not fit on an SM", h);
+  if (pl.res2_ok) {
+    h->res2_fn = res2_kernel(pl.comp, h->S.nat_eps != nullptr, pl.R2.P);
+    CUDA_OK(cudaFuncSetAttribute(h->res2_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->R2.smem_bytes));
+    CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->res2_fn, pl.res2_block, h->R2.smem_bytes));
+    if (occ < 1) return fail(SOP_E_CUDA, "the second resident kernel does not fit on an SM", h);
+  }
   if (R.C > 1) {
     int coop = 0, dev = 0;
     cudaGetDevice(&dev);
@@ -593,6 +719,7 @@ int resident_prepare(sop_handle *h) {
     if (!coop || (long long)h->S.T * R.C > (long long)occ * h->num_sms)
       return fail(SOP_E_CUDA, "the chunks of mode 3 cannot all be co-resident on this device", h);
     CUDA_OK(cudaMemsetAsync(R.xch, 0, 2 * (size_t)h->S.n_inst * 32, h->stream));
+    CUDA_OK(cudaMemsetAsync(R.xchf, 0, 2 * (size_t)h->S.n_inst * 32, h->stream));
   }
   CUDA_OK(cudaMemsetAsync(R.n_halo, 0, (size_t)h->S.T * R.C * 4, h->stream));
   return SOP_OK;
@@ -610,7 +737,12 @@ int resident_launch(sop_handle *h, int n, bool filter_last, bool filter_first) {
   uint32_t stamp0 = ((h->res_launch_id & 0xFFFu) << 20) | 1u;     // never 0, never the previous launch's stamps
   void *args[] = {&S, &R, &cur, &step0, &n, &nb, &fl, &stamp0};
   const dim3 grid((unsigned)(S.T * R.C)), block((unsigned)h->plan.res_block);
-  if (R.C > 1) CUDA_OK(cudaLaunchCooperativeKernel(h->res_fn, grid, block, args, (size_t)R.smem_bytes, h->stream));
+  if (h->plan.res2_ok) {
+    Res2Dev Q = h->R2;
+    void *args2[] = {&S, &R, &Q, &cur, &step0, &n, &nb, &fl, &stamp0};
+    CUDA_OK(cudaLaunchCooperativeKernel(h->res2_fn, grid, dim3((unsigned)h->plan.res2_block), args2, (size_t)Q.smem_bytes, h->stream));
+  }
+  else if (R.C > 1) CUDA_OK(cudaLaunchCooperativeKernel(h->res_fn, grid, block, args, (size_t)R.smem_bytes, h->stream));
   else CUDA_OK(cudaLaunchKernel(h->res_fn, grid, block, args, (size_t)R.smem_bytes, h->stream));
   h->launches++;
   return SOP_OK;
@@ -625,6 +757,10 @@ int rebuild_lists(sop_handle *h, bool with_filter = true) {
     const int loc_smem = ((h->S.N + 31) / 32) * 8 + h->R.chunk * 4;
     k_localise<<<(unsigned)(h->S.T * h->R.C), 1024, loc_smem, h->stream>>>(h->S, h->R);
     h->launches++;
+    if (h->plan.res2_ok) {
+      k_arrange_l1<<<(unsigned)(((long long)h->S.n_inst * 32 + 255) / 256), 256, 0, h->stream>>>(h->S, h->R, h->R2);
+      h->launches++;
+    }
   }
   if (with_filter) launch_filter(h);
   span_close(h);

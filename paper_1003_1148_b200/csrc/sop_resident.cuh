@@ -10,8 +10,17 @@
 // use) of its neighbours.  There is no grid barrier: every published 8-byte word carries (value, stamp), a reader
 // polls the words it needs until their stamps equal the step it is waiting for (64-bit accesses are single-copy
 // atomic), so a step costs one L2 round trip and a CTA only ever waits for the CTAs it really depends on.
-// Two exchange layers suffice: a CTA can only overwrite layer k with k+2 after it has read its neighbours'
-// layer k+1, which they publish after they finished reading layer k.
+// Readers and writers are kept apart by two pairs of layers.
+//  * step layers (parity of the step): read by ACTIVE readers only.  Being active is symmetric between chunks (bonds,
+//    natives and L2 rows are symmetric relations and both sides filter the same coordinates), so A overwrites stamp s
+//    with s+2 only after it has read B's stamp s+1, which B published after it finished reading A's stamp s.
+//  * filter layers (parity of step / nb_interval): the coordinates of the steps on which L2 is re-filtered (and of the
+//    launch prologue) are published here and nowhere else, and every chunk reads its WHOLE halo from them.  The L1
+//    relation is symmetric, so the same argument holds between any two chunks that are in each other's halo: A writes the
+//    filter layer of step s+2 nb only after reading C's layer of step s+nb, published after C finished reading step s.
+//    A halo-only (non-active) reader therefore never meets an overwritten slot, which a single pair of layers could not
+//    guarantee (a chunk only waits for its ACTIVE neighbours between filters).
+// Every wait is bounded (xch_wait): a protocol fault raises FLAG_EXCHANGE_TIMEOUT instead of hanging the launch.
 #pragma once
 #include <type_traits>
 
@@ -35,7 +44,10 @@ struct ResDev {
   int2 *bond_pack;            // [T*N][cap_b]     {slot or -1, bits(r0)} (C > 1)
   int2 *nat_T;                // one chunk, natives not in shared memory: the native table transposed, entry k of bead i
   int nat_tpad;               // at [k * nat_tpad + i], so that a warp of consecutive beads reads 256 contiguous bytes
-  uint4 *xch;                 // [2][T*N][2]  {x, stamp, y, stamp, z, stamp, -, -}: one 32-byte slot per bead
+  uint4 *xch;                 // [2][T*N][2]  step layers: one 32-byte slot {x|stamp, y|stamp, z|stamp, -} per bead and step parity
+  uint4 *xchf;                // [2][T*N][2]  filter layers: the coordinates of the steps on which L2 is re-filtered (read by the
+                              //              WHOLE halo), alternating with the parity of step / nb_interval
+  int skew_chunk, skew_period, skew_ns;   // test hook: chunk skew_chunk sleeps skew_ns before publishing on steps % skew_period == 0
   // shared-memory carve-up (bytes from the start of dynamic shared memory), computed by the host
   int off_pos, off_g, off_carry, off_tag, off_force, off_nb, off_cnt, off_plcnt, off_plofs, off_pl, off_natq,
       off_nat, off_bond, off_active, off_bm, off_sbm, off_misc, off_order, off_hist;
@@ -52,20 +64,41 @@ __device__ __forceinline__ float fast_rcp(float x) {
   return y;
 }
 
-// One 32-byte exchange slot per bead: {x, stamp, y, stamp, z, stamp, -, -}, written and read with ONE 256-bit access
-// (sm_100: LDG/STG.256) at gpu scope -- one L2 sector request per bead per poll instead of two.  Correctness only needs
-// each 8-byte {value, stamp} pair to be single-copy atomic (64-bit accesses are), so all three stamps are checked.
+// One 32-byte exchange slot per bead: three 64-bit elements {value, stamp} for x, y, z and one of padding, written and read
+// with ONE 256-bit access (sm_100: LDG/STG.256) at gpu scope -- one L2 sector request per bead per poll.  The PTX memory
+// model treats a vector access as one access per ELEMENT, so the elements are the 64-bit {value, stamp} pairs the
+// protocol needs to be single-copy atomic (.v4.b64), and all three stamps are checked.
 __device__ __forceinline__ void xch_put(uint4 *slot, const float4 &v, uint32_t st) {
-  asm volatile("st.relaxed.gpu.global.v8.u32 [%0], {%1, %2, %3, %2, %4, %2, %5, %5};" ::"l"(slot), "r"(__float_as_uint(v.x)),
-               "r"(st), "r"(__float_as_uint(v.y)), "r"(__float_as_uint(v.z)), "r"(0u) : "memory");
+  const unsigned long long hi = (unsigned long long)st << 32;
+  asm volatile("st.relaxed.gpu.global.v4.b64 [%0], {%1, %2, %3, %4};" ::"l"(slot), "l"(hi | __float_as_uint(v.x)),
+               "l"(hi | __float_as_uint(v.y)), "l"(hi | __float_as_uint(v.z)), "l"(0ull) : "memory");
 }
 
 __device__ __forceinline__ bool xch_try(const uint4 *slot, uint32_t st, float4 &out) {
-  uint32_t a0, a1, a2, a3, a4, a5, a6 = 0, a7 = 0;
-  asm volatile("ld.relaxed.gpu.global.v8.u32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-               : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3), "=r"(a4), "=r"(a5), "+r"(a6), "+r"(a7) : "l"(slot) : "memory");
-  out = make_float4(__uint_as_float(a0), __uint_as_float(a2), __uint_as_float(a4), 0.f);
-  return a1 == st && a3 == st && a5 == st;
+  unsigned long long a, b, c, d;
+  asm volatile("ld.relaxed.gpu.global.v4.b64 {%0, %1, %2, %3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(slot) : "memory");
+  out = make_float4(__uint_as_float((uint32_t)a), __uint_as_float((uint32_t)b), __uint_as_float((uint32_t)c), 0.f);
+  return (uint32_t)(a >> 32) == st && (uint32_t)(b >> 32) == st && (uint32_t)(c >> 32) == st;
+}
+
+// Bounded wait for one slot.  A CTA that waits longer than XCH_SPIN_LIMIT polls (seconds: a protocol fault, a dead
+// neighbour) raises FLAG_EXCHANGE_TIMEOUT and the abort word; every spinning thread looks at the abort word from time
+// to time and gives up too, so the cooperative launch ends with an error status instead of hanging the GPU.
+constexpr int FLAG_EXCHANGE_TIMEOUT = 32;
+constexpr unsigned XCH_SPIN_LIMIT = 1u << 23;
+__device__ __noinline__ bool xch_slow_wait(const uint4 *slot, uint32_t st, float4 &out, int *flags) {
+  volatile int *abort_word = flags + 1;
+  for (unsigned spins = 0;; ++spins) {
+    if (xch_try(slot, st, out)) return true;
+    if ((spins & 1023u) == 1023u) {
+      if (*abort_word) return false;
+      if (spins >= XCH_SPIN_LIMIT) { atomicOr(flags, FLAG_EXCHANGE_TIMEOUT); *abort_word = 1; __threadfence(); return false; }
+    }
+  }
+}
+__device__ __forceinline__ bool xch_wait(const uint4 *slot, uint32_t st, float4 &out, int *flags) {
+  if (xch_try(slot, st, out)) return true;
+  return xch_slow_wait(slot, st, out, flags);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -259,6 +292,8 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   const unsigned short DUMMY = (unsigned short)(SC - 1);
   const size_t inst0 = (size_t)t * S.N;
   uint4 *const xl0 = R.xch, *const xl1 = R.xch + 2 * (size_t)S.n_inst;
+  uint4 *const xf0 = R.xchf, *const xf1 = R.xchf + 2 * (size_t)S.n_inst;
+  unsigned fpar = (unsigned)((step0 / (unsigned long long)nb_interval) & 1ull);      // filter layer of the prologue
   const int cap_b = S.cap_b, cap_nb = S.cap_nb;
   const uint32_t traj = (uint32_t)(S.traj_offset + t);
   int flag = 0;
@@ -290,13 +325,13 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     const float4 v = S.pos[cur][inst0 + b0 + i];
     spos[i] = v;
     stag[i] = __float_as_uint(v.w);
-    if (multi) xch_put(xl0 + 2 * (inst0 + b0 + i), v, stamp0);
+    if (multi) xch_put((fpar ? xf1 : xf0) + 2 * (inst0 + b0 + i), v, stamp0);
     if (COMP) scarry[i] = S.carry[inst0 + b0 + i];
     natq[i] = S.nat_ptr[b0 + i];
     plcnt_s[i] = R.implicit_l1 ? (unsigned short)0 : (unsigned short)S.pl_cnt[inst0 + b0 + i];
     const uint32_t tag = __float_as_uint(v.w);
     if (G > 1 && !(tag & TAG_FIXED)) {
-      const float3 gn = gaussian3(S, tag & TAG_ID_MASK, traj, step0);
+      const float3 gn = S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step0);
       sg[i] = make_float4(gn.x, gn.y, gn.z, 0.f);
     }
   }
@@ -308,13 +343,14 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   if (R.nat_smem)
     for (int e = tid; e < n_nat; e += bd) snat[e] = nat_glob[qbase + e];
   const int2 *natp = R.nat_smem ? (const int2 *)snat - qbase : nat_glob;      // indexed by the global offset q
-  if (filter_first) {
-    // the launch starts on a fresh L1: the L2 rows come from Alg. 3 below, on the whole halo of the canonical layer
-    for (int q = tid; q < n_halo; q += bd) {
-      const float4 v = S.pos[cur][inst0 + hgid[q]];
-      spos[n_own + q] = make_float4(v.x, v.y, v.z, 0.f);
-    }
-  } else {
+  // the whole halo of the first layer comes through the exchange (never from S.pos, which a chunk that has finished a short
+  // launch overwrites in its epilogue while a late chunk is still in its prologue)
+  for (int q = tid; q < n_halo; q += bd) {
+    float4 v;
+    xch_wait((fpar ? xf1 : xf0) + 2 * (inst0 + hgid[q]), stamp0, v, S.flags);
+    spos[n_own + q] = v;
+  }
+  if (!filter_first) {
     for (int il = warp; il < n_own; il += nwarps) {
       const size_t g = inst0 + b0 + il;
       const int cnt = min(S.nb_cnt[g], cap_nb);
@@ -608,7 +644,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   K.k_fene = S.k_fene; K.inv_R0sq = S.inv_R0sq; K.eps12 = 12.0f * S.eps_native; K.c_rep_f = S.c_rep_f;
   const float *nat_eps = S.nat_eps;
   int until_filter = nb_interval - (int)(step0 % (unsigned long long)nb_interval);
-  bool have_full = filter_first;             // the whole halo of the current layer is already in shared memory
+  bool have_full = true;                     // the whole halo of the current layer is already in shared memory (prologue)
   for (int k = 0; k < n_steps; ++k) {
     const unsigned long long step = step0 + (unsigned long long)k;
     float4 *pc = spos + (size_t)(k & 1) * SC, *pn = spos + (size_t)((k & 1) ^ 1) * SC;
@@ -623,7 +659,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         const int slot = active[q];
         const uint4 *src = xc + 2 * (inst0 + hgid[slot - n_own]);
         float4 v;
-        while (!xch_try(src, st_c, v)) {}
+        xch_wait(src, st_c, v, S.flags);
         pc[slot] = v;
       }
     }
@@ -700,6 +736,10 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     SOP_SYNC();
     SOP_TICK(3)                                                                            // waiting for the slowest warp
     // (d2) a7 + a9: thread per bead; the other end of the block draws the next step's noise (a8)
+    const bool filt_due = until_filter == 1 && (k + 1 < n_steps || filter_last);   // the new layer is one every chunk filters on
+    if (filt_due) fpar ^= 1u;
+    uint4 *const xpub = filt_due ? (fpar ? xf1 : xf0) : xn;
+    if (R.skew_ns && tc == R.skew_chunk && step % (unsigned long long)R.skew_period == 0) __nanosleep((unsigned)R.skew_ns);
     for (int i = tid; i < n_own; i += bd) {
       const float4 ri = pc[i];
       const uint32_t tag = stag[i];
@@ -710,17 +750,17 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         external_force_at(S, b0 + i, ri, tag, ext, fx, fy, fz, flag);
         float3 gn;
         if (G > 1) { const float4 g4 = gc[i]; gn = make_float3(g4.x, g4.y, g4.z); }
-        else gn = gaussian3(S, tag & TAG_ID_MASK, traj, step);      // thread per bead already: nobody idles
+        else gn = S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step);   // thread per bead already
         out = langevin_apply<COMP>(S, ri, gn, fx, fy, fz, COMP ? scarry + i : nullptr, flag);
       }
       pn[i] = out;
-      if (multi) xch_put(xn + 2 * (inst0 + b0 + i), out, st_n);
+      if (multi) xch_put(xpub + 2 * (inst0 + b0 + i), out, st_n);
     }
     if (G > 1 && k + 1 < n_steps) {
       for (int i = bd - 1 - tid; i < n_own; i += bd) {
         const uint32_t tag = stag[i];
         if (!(tag & TAG_FIXED)) {
-          const float3 gn = gaussian3(S, tag & TAG_ID_MASK, traj, step + 1);
+          const float3 gn = S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step + 1);
           gnx[i] = make_float4(gn.x, gn.y, gn.z, 0.f);
         }
       }
@@ -732,9 +772,9 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
       if (k + 1 < n_steps || filter_last) {
         if (multi)
           for (int q = tid; q < n_halo; q += bd) {
-            const uint4 *src = xn + 2 * (inst0 + hgid[q]);
+            const uint4 *src = xpub + 2 * (inst0 + hgid[q]);
             float4 v;
-            while (!xch_try(src, st_n, v)) {}
+            xch_wait(src, st_n, v, S.flags);
             pn[n_own + q] = v;
           }
         __syncthreads();

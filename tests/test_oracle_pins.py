@@ -251,19 +251,44 @@ def test_p7_eq4_exact_without_noise():
 
 
 def test_p7_paper_parameters_error_bound():
-    """with the paper's own parameters the first-order recursion stays within the printed
-    relative error 2e-5 of Eq. (3) (evaluated here in closed form; 10^9 steps are not iterated)."""
+    """with the paper's own parameters (K_sp = 40 pN/nm, D = 1.5e-11 cm^2/s, h = 1, 25, 50 ps) the
+    ORACLE's update, iterated without noise, stays within the printed relative error 2e-5 of Eq. (3).  The paper's
+    harmonic particle under the ramp r_f t is the oracle's bead on a cantilever with kappa = K_sp, spring-base speed
+    v = r_f h / K_sp per step and h/xi = dt_over_zeta, so that kappa * dt_over_zeta = h/tau."""
     line = [l for l in open(os.path.join(GOLD, "eq3_eq4_paper_params.txt")) if not l.startswith("#")][0].split()
     Ksp, D_cm2s, kT, bound = float(line[0]), float(line[3]), float(line[4]), float(line[7])
     xi = kT / (D_cm2s * 1e14 * 1e-12)          # pN ps / nm   (D in nm^2/ps)
     tau = xi / Ksp                              # ps
+    n = 10 ** 6
+    for h in (1.0, 25.0, 50.0):
+        a = h / tau                             # = kappa * dt_over_zeta in the oracle's units
+        kappa = 1.0
+        w = gen.free_beads(2, R_pl=20.0, kT=0.0, pulled=[0, 1], pull_k=kappa, pull_v=1.0, pull_dir=[0.0, 0.0, 1.0])
+        p = dict(w.params, dt_over_zeta=a / kappa, nb_interval=1000, pl_interval=100000)
+        o = sopo.Oracle(w.xyz, w.bonds, w.native, p)
+        a = sopo.f32(a / kappa) * kappa         # the value the oracle really uses (parameters are fp32, promoted)
+        z0 = o.get_coords()[0, :, 2].copy()
+        o.run(n)
+        sim = (o.get_coords()[0, :, 2] - z0)    # in units of v = 1 per step
+        th = n - (1 - math.exp(-n * a)) / a     # Eq. (3) with X0 = 0, t = n h, in the same units
+        assert np.abs(sim - th).max() / th < bound
+        # and the closed form of the recursion X(n+1) = (1-a) X(n) + a n agrees with what the oracle iterated
+        closed = n - (1 - (1 - a) ** n) / a
+        assert np.abs(sim - closed).max() / closed < 1e-9
+
+
+def test_p7_mathematics_of_eq4_beyond_what_is_iterated():
+    """Mathematics only (no oracle call): the closed form of the first-order recursion Eq. (4) against Eq. (3) at the
+    paper's 10^8 and 10^9 steps, which are not iterated here."""
+    line = [l for l in open(os.path.join(GOLD, "eq3_eq4_paper_params.txt")) if not l.startswith("#")][0].split()
+    Ksp, D_cm2s, kT, bound = float(line[0]), float(line[3]), float(line[4]), float(line[7])
+    tau = kT / (D_cm2s * 1e14 * 1e-12) / Ksp
     for h in (1.0, 25.0, 50.0):
         a = h / tau
-        # closed form of X(n+1) = (1-a) X(n) + b n, X(0)=0:  X(n) = (b/a) (n - (1 - (1-a)^n)/a)
-        for n in (10 ** 6, 10 ** 8, 10 ** 9):
-            sim = (n - (1 - (1 - a) ** n) / a)              # in units of b/a
+        for n in (10 ** 8, 10 ** 9):
+            sim = (n - (1 - (1 - a) ** n) / a)
             t = n * h
-            th = (t - tau * (1 - math.exp(-t / tau))) / h   # same units
+            th = (t - tau * (1 - math.exp(-t / tau))) / h
             assert abs(sim - th) / th < bound
 
 
@@ -685,3 +710,31 @@ def test_p12_hybrid_taus_linearity_periods_lcg_and_moments():
     var = 2 * float(np.float32(0.6)) * float(np.float32(2e-3)) * nst
     assert abs(d.mean()) < 5 * math.sqrt(var / d.size)
     assert d.var() == pytest.approx(var, rel=5 * math.sqrt(2.0 / d.size))
+
+
+# ---------------------------------------------------------------------------------------------- P13
+def test_p13_eq1_magnitudes_two_beads_hand_evaluated():
+    """The VALUE of the native and repulsion terms away from their special points, with eps != 1: two beads on the x axis
+    against numbers evaluated by hand from Eq. (1) (tests/golden/eq1_two_bead_values.txt shows the arithmetic).
+    A wrong exponent (any n in (r0/r)^n passes P1 and P2), a wrong prefactor or a dropped eps fails here."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "eq1_two_bead_values.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 6
+    base = dict(gen.BASE_PARAMS, R_pl=math.inf, k_fene=14.0)
+    for term, eps, r0s, r, V, Fr in rows:
+        eps, r0s, r, V, Fr = float(eps), float(r0s), float(r), float(V), float(Fr)
+        if term == "native":
+            xyz = np.array([[0, 0, 0], [r0s, 0, 0]], np.float32)            # native distance = r0
+            p = dict(base, eps_native=eps, eps_rep=0.0)
+            o = sopo.Oracle(xyz, np.zeros((0, 2), np.int32), np.array([[0, 1]], np.int32), p)
+            col = 1
+        else:
+            xyz = np.array([[0, 0, 0], [5.0, 0, 0]], np.float32)            # inside R_nb: the pair is in L2
+            p = dict(base, eps_rep=eps, sigma=r0s, eps_native=0.0)
+            o = sopo.Oracle(xyz, np.zeros((0, 2), np.int32), np.zeros((0, 2), np.int32), p)
+            col = 2
+        e, f = o.eval_frozen(np.array([[0.0, 0, 0], [r, 0, 0]]))
+        tol = 2e-7                                                           # eps, sigma pass through fp32 (0.7, 3.8 are not exact)
+        assert e[col] == pytest.approx(V, rel=tol, abs=1e-12)
+        assert e[5] == pytest.approx(V, rel=tol, abs=1e-12)
+        assert f[1, 0] == pytest.approx(Fr, rel=tol, abs=1e-12) and f[0, 0] == pytest.approx(-Fr, rel=tol, abs=1e-12)
+        assert np.abs(f[:, 1:]).max() == 0.0
