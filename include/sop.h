@@ -83,10 +83,16 @@ typedef struct {
   int32_t reorder;                   /* 0 auto, 1 sort beads by native position inside the library, 2 keep order;
                                         invisible at the boundary (all indices in and out are the caller's) */
   int32_t chunk_beads;               /* mode 3: beads per chunk (one chunk per CTA); 0 auto */
+  int32_t resident_variant;          /* mode 3 with several chunks per trajectory: 0 auto (the faster one as measured, 1),
+                                        1 first design (lanes_per_bead lanes per bead, phases separated by block barriers),
+                                        2 second design (four lanes per bead, rows dealt by bank group, service warps that
+                                        overlap the exchange with the own-chunk partners) */
+  int32_t obs_stride, obs_capacity;  /* NEXT-1: record the observables + energies of every trajectory every obs_stride steps inside
+                                        sop_run into a DEVICE ring of obs_capacity samples (part of the workspace); 0, 0 = off */
   int32_t rng;                       /* 0 counter-based Philox4x32-10 (no generator state in memory); 1 the paper's Hybrid
                                         Taus (Alg. 6): 16 bytes of state per bead instance read and
-                                        written every step, seeded from Philox(seed); modes 1 and 2 only.  The state is
-                                        not part of sop_set_coords / sop_set_step, so an exact resume needs rng = 0 */
+                                        written every step, seeded from Philox(seed); every mode.  The state is not part
+                                        of sop_set_coords / sop_set_step, so an exact resume needs rng = 0 */
   void *stream;                      /* cudaStream_t */
 } sop_params;
 
@@ -120,6 +126,13 @@ int sop_get_energies(sop_handle *, double *e_out /*HOST [T][6]*/);
  * kappa (v s - (r_p - a_p).n)  (= r_f t at zero displacement, r_f = kappa v), o[3] = force resisting the
  * indenter sum_i F_i^tip . tip_dir.  fp32 terms, fp64 sums. */
 int sop_get_observables(sop_handle *, double *o_out /*HOST [T][4]*/);
+/* The series recorded inside sop_run (params.obs_stride): the curves of the paper's applications -- force-extension f(R)
+ * (PAPER.md:261), force-indentation (:312-314) -- and time averages without one host round trip per sample.
+ * A sample is taken whenever step % obs_stride == 0 after an update.  o_out: HOST [n][T][10] = {Rg, X, cantilever force, tip
+ * force, V_fene, V_nat, V_rep, V_pull, V_tip, V_total} of the last n <= max_samples samples, oldest first; steps_out: HOST [n]
+ * (may be NULL).  Synchronises.  sop_set_observable_stride changes the stride (0 = stop recording). */
+int sop_set_observable_stride(sop_handle *, int32_t stride);
+int sop_get_observable_series(sop_handle *, double *o_out, int64_t *steps_out, int32_t max_samples, int32_t *n_out);
 /* Deterministic force (no noise) at the current coordinates with the current L2, incl. external terms. */
 int sop_get_forces(sop_handle *, float *f_out /*HOST [T][N][3]*/);
 /* Row counts and rows (ascending caller index j, padded with -1 to cap) of trajectory traj.
@@ -132,8 +145,8 @@ int sop_set_step(sop_handle *, int64_t step);       /* with sop_set_coords: exac
  * perm_out (HOST [N], may be NULL) receives the caller index of each internal slot. */
 int sop_device_coords(sop_handle *, void **d_float4_out, int32_t *perm_out);
 /* What the auto settings resolved to: lanes_per_bead, block_size, compensated(0/1), mode(1/2/3), reorder(0/1),
- * cap_nb, cap_pl, kernel launches issued so far (lo, hi). */
-int sop_get_config(sop_handle *, int32_t out[9]);
+ * cap_nb, cap_pl, kernel launches issued so far (lo, hi), resident_variant in use (0 when the trajectory is one chunk). */
+int sop_get_config(sop_handle *, int32_t out[10]);
 /* Kernel timing for the bench (CUDA events on the handle's stream around groups of launches of one kind).
  * sop_get_profile synchronises, fills out[0..2] = ms spent in {step kernels, L2 filter kernels, L1 build kernels},
  * out[3..5] = number of timed spans of each kind, out[6] = Langevin steps covered by the step spans, and resets. */

@@ -34,7 +34,7 @@ struct Plan {                     // everything that depends only on (topology, 
   // workspace offsets
   size_t off_pos0, off_pos1, off_carry, off_force, off_bond, off_natptr, off_nattab, off_nateps, off_exclptr,
       off_exclidx, off_adotn, off_plcnt, off_plidx, off_nbcnt, off_nbidx, off_bbox, off_grid, off_cellof,
-      off_cellcnt, off_cellstart, off_cellbead, off_cellpos, off_taus, off_flags, off_epart, off_eout, off_bar, total;
+      off_cellcnt, off_cellstart, off_cellbead, off_cellpos, off_taus, off_flags, off_epart, off_eout, off_bar, off_series, total;
   // mode 3 (SM-resident kernel): chunking, launch shape, shared-memory carve-up, workspace
   bool res_ok = false;
   std::string res_why;
@@ -78,6 +78,9 @@ struct sop_handle {
  ResDev R;                       // mode 3
   Res2Dev R2;
   const void *res2_fn = nullptr;
+  int64_t obs_stride = 0, obs_count = 0;   // observables recorded every obs_stride steps into a device ring of obs_cap samples
+  int obs_cap = 0;
+  std::vector<int64_t> obs_steps;           // [obs_cap] step of the sample in every ring slot
   int obs_a = 0, obs_b = 0;       // internal indices of the two ends of the end-to-end distance
   const void *res_fn = nullptr;
   uint32_t res_launch_id = 0;
@@ -168,15 +171,16 @@ void plan_resident2(const sop_topology *tp, const sop_params *p, const std::vect
   Res2Dev &Q = pl.R2;
   memset(&Q, 0, sizeof(Q));
   pl.res2_ok = false;
-  if (R.C <= 1 || pl.static_l1 || getenv("SOP_TEST_OLD_RESIDENT")) return;
+  if (R.C <= 1 || pl.static_l1 || p->resident_variant != 2) return;     // (auto = the first design: measured faster)
   const int N = pl.N, chunk = R.chunk;
-  const int max_groups = (32 - R2_SERVICE_WARPS) * 4;
+  const int max_groups = (32 - 4) * 8;                          // groups of four lanes, at least four service warps
   const int P = (chunk + max_groups - 1) / max_groups;
-  if (P > R2_MAXP) return;
-  if ((p->lanes_per_bead != 0 && p->lanes_per_bead != 8) || p->block_size > 0) return;   // explicit launch shapes: first design
+  if (P > 2) return;                                             // (one or two beads per group: the filter keeps <= R2_MAXR rows per quarter-warp)
   Q.P = P;
-  Q.n_cwarps = (chunk + 4 * P - 1) / (4 * P);
-  pl.res2_block = 32 * (Q.n_cwarps + R2_SERVICE_WARPS);
+  Q.n_cwarps = (chunk + 8 * P - 1) / (8 * P);
+  Q.n_swarps = Q.n_cwarps <= 26 ? 6 : 32 - Q.n_cwarps;           // service warps: noise, exchange, bonds
+  pl.res2_block = 32 * (Q.n_cwarps + Q.n_swarps);
+  if ((chunk + pl.res2_block / 8 - 1) / (pl.res2_block / 8) > R2_MAXR) return;
   if (chunk > pl.res2_block || R.halo_cap > 32760 || pl.cap_pl > 496 || pl.cap_nb > 240 || pl.cap_b > 8) return;   // (15-bit partner codes, 64-bit survivor masks)
   Q.own_pad = (chunk + 7) / 8 * 8; Q.halo_pad = (R.halo_cap + 7) / 8 * 8;
   Q.own_stride = Q.own_pad + 8; Q.halo_stride = Q.halo_pad + 8;
@@ -195,7 +199,11 @@ void plan_resident2(const sop_topology *tp, const sop_params *p, const std::vect
     for (int i = 0; i < N; ++i) per[pl.iperm[i] / chunk] += nnb[i] + nnat[i] + 8;
   }
   long long want = (long long)(*std::max_element(per.begin(), per.end()) * 1.15) + 64;
-  want = std::min<long long>((want + 7) / 8 * 8, 65528LL * 8);
+  want = std::max<long long>(2048, std::min<long long>((want + 7) / 8 * 8, 65528LL * 4));      // (>= 8 KB: scratch of the prologue)
+  {   // the prologue of a launch that continues on an old L1 keeps one membership bitmap per quarter-warp in the row region
+    const long long bm_bytes = (long long)(pl.res2_block / 8) * ((Q.own_stride + Q.halo_stride + 31) / 32) * 4;
+    want = std::max<long long>(want, (bm_bytes / 8 + 8) / 8 * 8);
+  }
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = (o + bytes + 127) / 128 * 128; return (int)at; };
   auto carve = [&](long long rows_cap) {
@@ -205,7 +213,6 @@ void plan_resident2(const sop_topology *tp, const sop_params *p, const std::vect
     Q.off_halo = take(2 * (size_t)Q.halo_stride * 16);
     Q.off_rows = take((size_t)rows_cap * 8);
     Q.off_eps = take(tp->native_eps ? (size_t)rows_cap * 4 : 0);
-    Q.off_kbase = take((size_t)chunk * 16);
     Q.off_ext = take(32);
     Q.off_g = take(2 * (size_t)chunk * 16);
     Q.off_carry = take(pl.comp ? (size_t)chunk * 16 : 0);
@@ -213,16 +220,16 @@ void plan_resident2(const sop_topology *tp, const sop_params *p, const std::vect
     Q.off_rowofs = take(((size_t)chunk + 1) * 2);
     Q.off_rowg = take((size_t)chunk * 2);
     Q.off_nat = take((size_t)R.nat_cap * 8);
+    Q.off_nateps = take(tp->native_eps ? (size_t)R.nat_cap * 4 : 0);
     Q.off_natq = take(((size_t)chunk + 1) * 4);
+    Q.off_natc = take((size_t)chunk * 2);
     Q.off_bond = take((size_t)chunk * pl.cap_b * 8);
-    Q.off_tmp = take((size_t)chunk * pl.cap_nb * 2);
     Q.off_cnt = take((size_t)chunk * 2);
     Q.off_active = take((size_t)R.halo_cap * 2);
     Q.off_bm = take((size_t)(R.halo_cap / 32 + 1) * 4);
     Q.off_sbm = take((size_t)(R.halo_cap / 32 + 1) * 4);
-    Q.off_misc = take(64);
-    Q.off_order = take((size_t)chunk * 2);
-    Q.off_hist = take((size_t)std::max(64, (pl.res2_block / 32) * 64) * 4);
+    Q.off_misc = take(2048);
+    Q.off_order = take((size_t)chunk * 4);
     Q.off_taus = take(p->rng == 1 ? (size_t)chunk * 16 : 0);
     Q.smem_bytes = (int)o;
   };
@@ -237,7 +244,7 @@ void plan_resident2(const sop_topology *tp, const sop_params *p, const std::vect
   if (o > 232448) {                       // the rows get what is left, if that is still most of what they may need
     const long long fixed = (long long)o - want * per_entry;
     const long long left = (232448 - fixed - 512) / per_entry / 8 * 8;
-    if (left * 10 < want * 8) return;
+    if (left * 10 < want * 8 || left < 2048 || left * 8 < (long long)(pl.res2_block / 8) * ((Q.own_stride + Q.halo_stride + 31) / 32) * 4) return;
     carve(left);
     if (o > 232448) return;
   }
@@ -448,6 +455,9 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.block = p->block_size > 0 ? p->block_size : 256;
   if (pl.block % 32 || pl.block > 1024) return fail(SOP_E_ARG, "block_size must be a multiple of 32, <= 1024");
   if (p->mode < 0 || p->mode > 3) return fail(SOP_E_ARG, "mode must be 0, 1, 2 or 3");
+  if (p->obs_stride < 0 || p->obs_capacity < 0 || (p->obs_stride > 0 && p->obs_capacity < 1))
+    return fail(SOP_E_ARG, "obs_stride needs obs_capacity >= 1");
+  if (p->resident_variant < 0 || p->resident_variant > 2) return fail(SOP_E_ARG, "resident_variant must be 0, 1 or 2");
   if (p->rng != 0 && p->rng != 1) return fail(SOP_E_ARG, "rng must be 0 (Philox) or 1 (Hybrid Taus)");
   pl.mode = p->mode;
   if (pl.mode == 0 || pl.mode == 3) {
@@ -486,6 +496,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.off_epart = take((size_t)T * pl.energy_blocks * 5 * 8);
   pl.off_eout = take((size_t)T * 6 * 8);
   pl.off_bar = take(256);
+  pl.off_series = take(p->obs_capacity > 0 ? (size_t)p->obs_capacity * T * 10 * 8 : 0);
   if (pl.mode == 3) {
     const ResDev &R = pl.R;
     const bool multi = R.C > 1;
@@ -667,12 +678,7 @@ const void *resident_kernel(int lanes, bool comp) {
 
 template <bool COMP, bool EPS>
 const void *res2_fn_p(int P) {
-  switch (P) {
-    case 1: return (const void *)k_res2<COMP, EPS, 1>;
-    case 2: return (const void *)k_res2<COMP, EPS, 2>;
-    case 3: return (const void *)k_res2<COMP, EPS, 3>;
-    default: return (const void *)k_res2<COMP, EPS, 4>;
-  }
+  return P == 1 ? (const void *)k_res2<COMP, EPS, 1> : (const void *)k_res2<COMP, EPS, 2>;
 }
 const void *res2_kernel(bool comp, bool eps, int P) {
   if (comp) return eps ? res2_fn_p<true, true>(P) : res2_fn_p<true, false>(P);
@@ -765,6 +771,25 @@ int rebuild_lists(sop_handle *h, bool with_filter = true) {
   if (with_filter) launch_filter(h);
   span_close(h);
   return check_launch(h, "list rebuild");
+}
+
+
+// NEXT-1: one sample of the observable series = {Rg, X, cantilever force, tip force, V_fene, V_nat, V_rep, V_pull, V_tip, -}
+// per trajectory, reduced on the device into slot (count mod capacity) of the ring; nothing goes to the host.
+int record_sample(sop_handle *h) {
+  const SysDev &S = h->S;
+  const int slot = (int)(h->obs_count % h->obs_cap);
+  double *d_slot = (double *)(h->ws + h->plan.off_series) + (size_t)slot * S.T * 10;
+  double *partial = (double *)(h->ws + h->plan.off_epart);
+  span_close(h);
+  k_observables<<<(unsigned)S.T, 1024, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, h->obs_a, h->obs_b, d_slot, 10);
+  dim3 grid((unsigned)h->plan.energy_blocks, (unsigned)S.T);
+  k_energy<<<grid, 256, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, partial);
+  k_energy_final<<<(S.T * 5 + 127) / 128, 128, 0, h->stream>>>(S.T, h->plan.energy_blocks, partial, d_slot + 4, 10);
+  h->launches += 3;
+  h->obs_steps[slot] = h->step;
+  h->obs_count++;
+  return check_launch(h, "observable sample");
 }
 
 }  // namespace
@@ -957,6 +982,8 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
     h->launches++;
   }
   h->cur = 0; h->step = 0;
+  h->obs_stride = p->obs_capacity > 0 ? p->obs_stride : 0; h->obs_cap = p->obs_capacity;
+  h->obs_steps.assign((size_t)std::max(0, p->obs_capacity), 0);
   rc = rebuild_lists(h);
   if (!rc) rc = read_flags(h);
   if (rc) { std::string m = h->last_error; delete h; return fail(rc, m); }
@@ -1001,37 +1028,71 @@ int sop_get_profile(sop_handle *h, double out[8]) {
 
 int sop_run(sop_handle *h, int64_t n_steps) {
   if (!h || n_steps < 0) return fail(SOP_E_ARG, "bad handle or n_steps", h);
-  const int64_t nb = h->prm.nb_interval, plv = h->prm.pl_interval;
+  const int64_t nb = h->prm.nb_interval, plv = h->prm.pl_interval, ost = h->obs_stride;
   int64_t left = n_steps;
   bool pending_filter = false;
   while (left > 0) {
     if (h->plan.mode >= 2) {
-      // one persistent launch runs up to the next pair-list boundary, re-filtering L2 inside
+      // one persistent launch runs up to the next pair-list boundary (or observable sample), re-filtering L2 inside
       int64_t n = std::min<int64_t>(left, (1 << 20) - 2);
       if (!h->S.static_l1) n = std::min<int64_t>(n, plv - (h->step % plv));
+      if (ost > 0) n = std::min<int64_t>(n, ost - (h->step % ost));
       const bool l1_due = !h->S.static_l1 && (h->step + n) % plv == 0;
+      const bool sample_due = ost > 0 && (h->step + n) % ost == 0;
       int rc = h->plan.mode == 3 ? resident_launch(h, (int)n, !l1_due, pending_filter) : persistent_launch(h, (int)n, !l1_due);
       if (rc) return rc;
       pending_filter = false;
       if (h->plan.mode == 2) h->cur ^= (int)(n & 1);      // mode 3 writes the final layer back in place
       h->step += n; left -= n;
       if (l1_due) {
-        pending_filter = h->plan.mode == 3 && left > 0;
+        // (a sample needs the canonical L2 of this very step: the filter then runs as its own kernel)
+        pending_filter = h->plan.mode == 3 && left > 0 && !sample_due;
         rc = rebuild_lists(h, !pending_filter);
         if (rc) return rc;
         if (pending_filter) h->l2_built_at = h->step;
       }
       else if (h->step / nb * nb > h->l2_built_at) h->l2_built_at = h->step / nb * nb;
+      if (sample_due) { rc = record_sample(h); if (rc) return rc; }
     } else {
       span_begin(h, SPAN_STEP, 1);
       launch_step(h, false);
       h->cur ^= 1; h->step++; left--;
       if (!h->S.static_l1 && h->step % plv == 0) { int rc = launch_build_l1(h); if (rc) return rc; }
       if (h->step % nb == 0) launch_filter(h);
+      if (ost > 0 && h->step % ost == 0) { int rc = record_sample(h); if (rc) return rc; }
     }
   }
   span_close(h);
   return check_launch(h, "sop_run");
+}
+
+int sop_set_observable_stride(sop_handle *h, int32_t stride) {
+  if (!h || stride < 0) return fail(SOP_E_ARG, "bad stride", h);
+  if (stride > 0 && h->obs_cap < 1) return fail(SOP_E_ARG, "the handle was created with obs_capacity = 0", h);
+  h->obs_stride = stride;
+  return SOP_OK;
+}
+
+int sop_get_observable_series(sop_handle *h, double *o_out, int64_t *steps_out, int32_t max_samples, int32_t *n_out) {
+  if (!h || !n_out || max_samples < 0) return fail(SOP_E_ARG, "null argument", h);
+  const int T = h->S.T;
+  const int64_t have = std::min<int64_t>(h->obs_count, h->obs_cap);
+  const int n = (int)std::min<int64_t>(have, max_samples);
+  *n_out = n;
+  if (n == 0) return read_flags(h);
+  if (!o_out) return fail(SOP_E_ARG, "o_out is null", h);
+  const double *ring = (const double *)(h->ws + h->plan.off_series);
+  for (int q = 0; q < n; ++q) {                 // the last n samples, oldest first
+    const int slot = (int)((h->obs_count - n + q) % h->obs_cap);
+    CUDA_OK(cudaMemcpyAsync(o_out + (size_t)q * T * 10, ring + (size_t)slot * T * 10, (size_t)T * 80, cudaMemcpyDeviceToHost, h->stream));
+    if (steps_out) steps_out[q] = h->obs_steps[slot];
+  }
+  int rc = read_flags(h);
+  for (size_t r = 0; r < (size_t)n * T; ++r) {
+    double *e = o_out + 10 * r + 4;
+    e[5] = e[0] + e[1] + e[2] + e[3] + e[4];
+  }
+  return rc;
 }
 
 int sop_sync(sop_handle *h) {
@@ -1098,7 +1159,7 @@ int sop_get_energies(sop_handle *h, double *e_out) {
   double *partial = (double *)(h->ws + h->plan.off_epart), *d_e = (double *)(h->ws + h->plan.off_eout);
   dim3 grid((unsigned)h->plan.energy_blocks, (unsigned)S.T);
   k_energy<<<grid, 256, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, partial);
-  k_energy_final<<<(S.T * 5 + 127) / 128, 128, 0, h->stream>>>(S.T, h->plan.energy_blocks, partial, d_e);
+  k_energy_final<<<(S.T * 5 + 127) / 128, 128, 0, h->stream>>>(S.T, h->plan.energy_blocks, partial, d_e, 6);
   h->launches += 2;
   int rc = check_launch(h, "energy");
   if (rc) return rc;
@@ -1115,7 +1176,7 @@ int sop_get_observables(sop_handle *h, double *o_out) {
   if (!h || !o_out) return fail(SOP_E_ARG, "null argument", h);
   const SysDev &S = h->S;
   double *d_o = (double *)(h->ws + h->plan.off_epart);          // reuses the energy partial buffer (>= T * 40 bytes)
-  k_observables<<<(unsigned)S.T, 1024, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, h->obs_a, h->obs_b, d_o);
+  k_observables<<<(unsigned)S.T, 1024, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, h->obs_a, h->obs_b, d_o, 4);
   h->launches++;
   int rc = check_launch(h, "observables");
   if (rc) return rc;
@@ -1189,11 +1250,13 @@ extern "C" int sop_debug_phase_clocks(sop_handle *h, float *out, int n_float4) {
 }
 #endif
 
-int sop_get_config(sop_handle *h, int32_t out[9]) {
+int sop_get_config(sop_handle *h, int32_t out[10]) {
   if (!h || !out) return fail(SOP_E_ARG, "null argument", h);
   out[0] = h->plan.mode == 3 ? h->plan.res_lanes : h->plan.lanes; out[1] = h->plan.mode == 3 ? h->plan.res_block : h->plan.block; out[2] = h->plan.comp; out[3] = h->plan.mode;
   out[4] = h->plan.reorder; out[5] = h->plan.cap_nb; out[6] = h->plan.cap_pl;
   out[7] = (int32_t)(h->launches & 0xFFFFFFFFu); out[8] = (int32_t)(h->launches >> 32);
+  out[9] = h->plan.mode == 3 && h->R.C > 1 ? (h->plan.res2_ok ? 2 : 1) : 0;
+  if (out[9] == 2) { out[0] = R2_GS; out[1] = h->plan.res2_block; }
   return SOP_OK;
 }
 

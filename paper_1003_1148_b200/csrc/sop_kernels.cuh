@@ -423,7 +423,7 @@ __device__ __forceinline__ double block_sum(double v, double *red) {
   return tot;
 }
 
-__global__ void __launch_bounds__(1024) k_observables(SysDev S, int cur, unsigned long long step, int ia, int ib, double *o_out) {
+__global__ void __launch_bounds__(1024) k_observables(SysDev S, int cur, unsigned long long step, int ia, int ib, double *o_out, int o_stride) {
   __shared__ double red[32];
   const int t = blockIdx.x;
   const float4 *__restrict__ pos_t = S.pos[cur] + (size_t)t * S.N;
@@ -461,19 +461,19 @@ __global__ void __launch_bounds__(1024) k_observables(SysDev S, int cur, unsigne
   if (threadIdx.x == 0) {
     const float4 a = pos_t[ia], b = pos_t[ib];
     const double dx = (double)b.x - (double)a.x, dy = (double)b.y - (double)a.y, dz = (double)b.z - (double)a.z;
-    double *o = o_out + 4 * (size_t)t;
+    double *o = o_out + (size_t)o_stride * (size_t)t;
     o[0] = sqrt(s2 / n); o[1] = sqrt(dx * dx + dy * dy + dz * dz); o[2] = fp; o[3] = ft;
   }
   if (flag) atomicOr(S.flags, flag);
 }
 
-__global__ void k_energy_final(int T, int nblk, const double *partial, double *e_out) {
+__global__ void k_energy_final(int T, int nblk, const double *partial, double *e_out, int e_stride) {
   int q = blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= T * 5) return;
   int t = q / 5, k = q % 5;
   double v = 0;
   for (int b = 0; b < nblk; ++b) v += partial[((size_t)t * nblk + b) * 5 + k];
-  e_out[t * 6 + k] = v;
+  e_out[(size_t)t * e_stride + k] = v;
 }
 
 }  // namespace sop

@@ -16,7 +16,8 @@ STATUS = {0: "SOP_OK", -1: "SOP_E_ARG", -2: "SOP_E_CUDA", -3: "SOP_E_LIST_OVERFL
 
 SYMBOLS = ["sop_query_workspace", "sop_create", "sop_destroy", "sop_run", "sop_sync", "sop_get_coords",
            "sop_set_coords", "sop_get_energies", "sop_get_observables", "sop_get_forces", "sop_get_lists", "sop_get_step", "sop_set_step",
-           "sop_device_coords", "sop_get_config", "sop_set_profiling", "sop_get_profile", "sop_last_error"]
+           "sop_device_coords", "sop_get_config", "sop_set_profiling", "sop_get_profile", "sop_last_error",
+           "sop_set_observable_stride", "sop_get_observable_series"]
 
 
 class _Topology(C.Structure):
@@ -41,7 +42,8 @@ class _Params(C.Structure):
                 ("tip_on", C.c_int32), ("tip_R", C.c_float), ("tip_eps", C.c_float), ("tip_sigma", C.c_float),
                 ("tip_c0", C.c_float * 3), ("tip_dir", C.c_float * 3), ("tip_v", C.c_float),
                 ("lanes_per_bead", C.c_int32), ("block_size", C.c_int32), ("compensated", C.c_int32),
-                ("mode", C.c_int32), ("reorder", C.c_int32), ("chunk_beads", C.c_int32), ("rng", C.c_int32),
+                ("mode", C.c_int32), ("reorder", C.c_int32), ("chunk_beads", C.c_int32), ("resident_variant", C.c_int32),
+                ("obs_stride", C.c_int32), ("obs_capacity", C.c_int32), ("rng", C.c_int32),
                 ("stream", C.c_void_p)]
 
 
@@ -70,6 +72,8 @@ def lib():
         L.sop_get_energies.argtypes = [vp, vp]
         L.sop_get_forces.argtypes = [vp, vp]
         L.sop_get_observables.argtypes = [vp, vp]
+        L.sop_set_observable_stride.argtypes = [vp, i32]
+        L.sop_get_observable_series.argtypes = [vp, vp, vp, i32, C.POINTER(i32)]
         L.sop_get_lists.argtypes = [vp, i32, i32, vp, vp, C.POINTER(i32), C.POINTER(i64)]
         L.sop_get_step.argtypes = [vp, C.POINTER(i64)]
         L.sop_set_step.argtypes = [vp, i64]
@@ -125,6 +129,8 @@ def _marshal(xyz, bonds, native, params, native_eps, overrides):
     pp.lanes_per_bead = int(p.get("lanes_per_bead", 0)); pp.block_size = int(p.get("block_size", 0))
     pp.compensated = int(p.get("compensated", 0)); pp.mode = int(p.get("mode", 0)); pp.reorder = int(p.get("reorder", 0))
     pp.chunk_beads = int(p.get("chunk_beads", 0)); pp.rng = int(p.get("rng", 0))
+    pp.resident_variant = int(p.get("resident_variant", 0))
+    pp.obs_stride = int(p.get("obs_stride", 0)); pp.obs_capacity = int(p.get("obs_capacity", 0))
     return tp, pp, keep
 
 
@@ -141,6 +147,7 @@ class Sop:
         self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
         tp, pp, self._keep = _marshal(xyz, bonds, native, params, native_eps, overrides)
         self.N = tp.n_beads; self.T = int(n_traj)
+        self._keep_obs_capacity = pp.obs_capacity
         with torch.cuda.device(self.device):
             self._stream = torch.cuda.current_stream()
             pp.stream = self._stream.cuda_stream
@@ -194,6 +201,17 @@ class Sop:
         self._chk(lib().sop_get_observables(self._h, out.ctypes.data), "sop_get_observables")
         return out
 
+    def set_observable_stride(self, stride):
+        self._chk(lib().sop_set_observable_stride(self._h, int(stride)), "sop_set_observable_stride")
+
+    def get_observable_series(self, max_samples=1 << 20):
+        """-> (steps[n], series[n][T][10]): Rg, X, cantilever force, tip force, V_fene, V_nat, V_rep, V_pull, V_tip, V_total
+        of the samples recorded inside run() every obs_stride steps (the last `obs_capacity` of them at most)."""
+        cap = max(1, min(int(max_samples), int(self._keep_obs_capacity)))
+        out = np.zeros((cap, self.T, 10), np.float64); steps = np.zeros(cap, np.int64); n = C.c_int32()
+        self._chk(lib().sop_get_observable_series(self._h, out.ctypes.data, steps.ctypes.data, cap, C.byref(n)), "sop_get_observable_series")
+        return steps[:n.value].copy(), out[:n.value].copy()
+
     def set_coords(self, xyz):
         x = np.ascontiguousarray(xyz, np.float32).reshape(self.T, self.N, 3)
         self._chk(lib().sop_set_coords(self._h, x.ctypes.data), "sop_set_coords")
@@ -221,11 +239,12 @@ class Sop:
         self._chk(lib().sop_set_step(self._h, int(v)), "sop_set_step")
 
     def config(self):
-        out = np.zeros(9, np.int32)
+        out = np.zeros(10, np.int32)
         self._chk(lib().sop_get_config(self._h, out.ctypes.data), "sop_get_config")
         names = ["lanes_per_bead", "block_size", "compensated", "mode", "reorder", "cap_nb", "cap_pl"]
         d = {k: int(v) for k, v in zip(names, out[:7])}
         d["launches"] = int(np.uint32(out[7])) | (int(np.uint32(out[8])) << 32)
+        d["resident_variant"] = int(out[9])
         return d
 
     def set_profiling(self, on=True):
@@ -261,6 +280,8 @@ def sop_set_coords(h, xyz): return h.set_coords(xyz)
 def sop_get_energies(h): return h.get_energies()
 def sop_get_forces(h): return h.get_forces()
 def sop_get_observables(h): return h.get_observables()
+def sop_set_observable_stride(h, stride): return h.set_observable_stride(stride)
+def sop_get_observable_series(h, max_samples=1 << 20): return h.get_observable_series(max_samples)
 def sop_get_lists(h, level, traj=0): return h.get_lists(level, traj)
 def sop_get_step(h): return h.step
 def sop_set_step(h, v): h.step = v

@@ -75,7 +75,8 @@ SMALL = [
 VARIANTS = [dict(mode=1, lanes_per_bead=1), dict(mode=1, lanes_per_bead=8), dict(mode=1, lanes_per_bead=32),
             dict(mode=2, lanes_per_bead=4), dict(mode=2, lanes_per_bead=16, reorder=1), dict(mode=1, reorder=1),
             dict(mode=3), dict(mode=3, chunk_beads=40, lanes_per_bead=4), dict(mode=3, chunk_beads=64, lanes_per_bead=1),
-            dict(mode=3, chunk_beads=33, lanes_per_bead=16, compensated=1)]
+            dict(mode=3, chunk_beads=33, lanes_per_bead=16, compensated=1),
+            dict(mode=3, chunk_beads=40, resident_variant=2), dict(mode=3, chunk_beads=64, resident_variant=2, compensated=1)]
 
 
 @pytest.mark.parametrize("name,make,over", SMALL, ids=[c[0] for c in SMALL])
@@ -138,7 +139,7 @@ def test_run_split_variant_and_mode_independence():
     assert np.abs(c.get_coords() - ref).max() < 1e-4       # other summation order: fp32 rounding only
     # the SM-resident kernel: bit-identical however the run is split and whatever else ran before on the exchange
     # buffer; against the streaming kernels only the rounding of the pair terms differs
-    for var in (dict(mode=3), dict(mode=3, chunk_beads=48, lanes_per_bead=8)):
+    for var in (dict(mode=3), dict(mode=3, chunk_beads=48, lanes_per_bead=8), dict(mode=3, chunk_beads=48, resident_variant=2)):
         a = sop().from_workload(w, **var); a.run(130)
         b = sop().from_workload(w, **var); b.run(7); b.run(93); b.run(1); b.run(29)
         assert a.config()["mode"] == 3
@@ -150,7 +151,7 @@ def test_run_split_variant_and_mode_independence():
         assert np.abs(a.get_coords() - ref).max() < 1e-4
 
 
-@pytest.mark.parametrize("var", [dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=40)], ids=str)
+@pytest.mark.parametrize("var", [dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=40), dict(mode=3, chunk_beads=40, resident_variant=2)], ids=str)
 def test_checkpoint_resume_is_exact(var):
     w = gen.tiny(128, 9, R_pl=20.0)
     a = sop().from_workload(w, **var); a.run(300)
@@ -160,7 +161,8 @@ def test_checkpoint_resume_is_exact(var):
     assert np.array_equal(a.get_coords(), c.get_coords())
 
 
-@pytest.mark.parametrize("var", [dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=32, R_pl=20.0)], ids=str)
+@pytest.mark.parametrize("var", [dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=32, R_pl=20.0),
+                                 dict(mode=3, chunk_beads=32, R_pl=20.0, resident_variant=2)], ids=str)
 def test_batch_trajectories_and_sharding_offset(var):
     var = dict(var)
     w = gen.tiny(96, 4, **({"R_pl": var.pop("R_pl")} if "R_pl" in var else {}))
@@ -326,16 +328,18 @@ def test_full_config1_batch_finite_pair_list():
         check_lists(s, o, xg[t], traj=t)
 
 
-@pytest.mark.parametrize("mode", [2, 3])
-def test_full_config2_fiber_pulled(mode):
-    s = full_check(2, mode=mode)
+@pytest.mark.parametrize("mode,variant", [(2, 0), (3, 1), (3, 2)])
+def test_full_config2_fiber_pulled(mode, variant):
+    s = full_check(2, mode=mode, resident_variant=variant)
     assert s.config()["compensated"] == 1 and s.config()["mode"] == mode
+    assert variant == 0 or s.config()["resident_variant"] == variant
 
 
-@pytest.mark.parametrize("mode", [1, 2, 3])
-def test_full_config3_shell_indented(mode):
-    s = full_check(3, mode=mode)
+@pytest.mark.parametrize("mode,variant", [(1, 0), (2, 0), (3, 1), (3, 2)])
+def test_full_config3_shell_indented(mode, variant):
+    s = full_check(3, mode=mode, resident_variant=variant)
     assert s.config()["mode"] == mode
+    assert variant == 0 or s.config()["resident_variant"] == variant
 
 
 @pytest.mark.parametrize("mode", [0, 1])
@@ -344,8 +348,8 @@ def test_full_config4_lattice(mode):
 
 
 # ---------------------------------------------------------------------------------------------- more mode-3 coverage
-@pytest.mark.parametrize("var", [dict(mode=1, lanes_per_bead=4), dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=45)],
-                         ids=str)
+@pytest.mark.parametrize("var", [dict(mode=1, lanes_per_bead=4), dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=45),
+                                 dict(mode=3, chunk_beads=45, resident_variant=2)], ids=str)
 def test_per_contact_native_eps(var):
     """topology.native_eps (one eps per native contact, PAPER.md:241 eps_n) on every kernel path."""
     w = gen.tiny(150, 21, R_pl=20.0)
@@ -358,16 +362,27 @@ def test_per_contact_native_eps(var):
     assert np.abs(s.get_coords() - o.get_coords()).max() <= 1e-3
 
 
-def test_mode3_long_run_across_pair_list_rebuilds():
+@pytest.mark.parametrize("var", [dict(mode=1), dict(mode=2), dict(mode=3, chunk_beads=60), dict(mode=3, chunk_beads=60, resident_variant=2)], ids=str)
+def test_mode3_long_run_across_pair_list_rebuilds(var):
     """350 steps = 3 pair-list rebuilds inside one sop_run (the in-kernel first filter after each) against three
     separate runs that end on the rebuild boundaries (k_filter path) and against the oracle's lists at the end."""
     w = gen.two_chains(150, 3, R_pl=20.0)
-    a = sop().from_workload(w, mode=3, chunk_beads=60); a.run(350)
-    b = sop().from_workload(w, mode=3, chunk_beads=60); b.run(100); b.run(200); b.run(50)
+    a = sop().from_workload(w, **var); a.run(350)
+    b = sop().from_workload(w, **var); b.run(100); b.run(200); b.run(50)
     assert np.array_equal(a.get_coords(), b.get_coords())
     o = sopo.from_workload(w)
     xa = a.get_coords()
     assert a.get_lists(1)[2] == 300 and a.get_lists(2)[2] == 350
+    # the L2 of step 350 is Alg. 3 applied to the STALE L1 of step 300 at the coordinates of step 350: bit for bit the
+    # oracle's filter of the GPU's own L1 (a fresh build at step 350 would give a different list)
+    c1, i1, _ = a.get_lists(1)
+    c2, i2, _ = a.get_lists(2)
+    oc, oi = o.filter(xa[0].astype(np.float64), c1, i1)
+    assert np.array_equal(c2, oc)
+    for i in range(w.n_beads):
+        assert np.array_equal(i2[i, :c2[i]], oi[i, :oc[i]])
+    fc, fi = o.build_lists(xa[0].astype(np.float64), 1, cap=i1.shape[1])
+    assert not np.array_equal(fc, c1)                          # the pair list really is stale
     # L2 was filtered at step 350 from the L1 of step 300: compare with the oracle driven to the same state
     o.run(350)
     assert np.abs(xa - o.get_coords()).max() <= 5e-3          # 350 steps: fp32 vs fp64 drift, still far below a bond length
@@ -417,7 +432,8 @@ def check_observables(s, o, xg, step):
     assert (np.abs(got - ref) <= 2e-5 * scale + 1e-6).all(), (got, ref)     # fp32 coordinates and terms, fp64 sums
 
 
-@pytest.mark.parametrize("var", [dict(mode=1), dict(mode=3), dict(mode=3, chunk_beads=24, R_pl=20.0)], ids=str)
+@pytest.mark.parametrize("var", [dict(mode=1), dict(mode=3), dict(mode=3, chunk_beads=24, R_pl=20.0),
+                                 dict(mode=3, chunk_beads=24, R_pl=20.0, resident_variant=2)], ids=str)
 def test_observables_small_with_pull_and_tip(var):
     var = dict(var)
     w = gen.tiny(64, 8)
@@ -460,7 +476,8 @@ def test_mode3_is_deterministic_run_to_run():
     SM-resident kernel must give bit-identical coordinates, lists and energies every time, on small chunked systems
     (many exchange partners per CTA) and on the full 30,000-bead shell with all 148 CTAs polling each other."""
     w = gen.two_chains(150, 3, R_pl=20.0)
-    for var in (dict(chunk_beads=30, lanes_per_bead=8), dict(chunk_beads=75, lanes_per_bead=1), dict(n_traj=3, chunk_beads=50)):
+    for var in (dict(chunk_beads=30, lanes_per_bead=8), dict(chunk_beads=75, lanes_per_bead=1), dict(n_traj=3, chunk_beads=50),
+                dict(n_traj=3, chunk_beads=50, resident_variant=2)):
         var = dict(var); T = var.pop("n_traj", 1)
         ref = None
         for rep in range(4):
@@ -482,7 +499,8 @@ def test_mode3_is_deterministic_run_to_run():
             assert np.array_equal(ref, x), rep
 
 
-@pytest.mark.parametrize("var", [dict(mode=1), dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=40)], ids=str)
+@pytest.mark.parametrize("var", [dict(mode=1), dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=40),
+                                 dict(mode=3, chunk_beads=40, resident_variant=2)], ids=str)
 def test_a_blown_up_structure_reports_errors_but_stays_memory_safe(var):
     """A caller that ignores SOP_E_FENE / SOP_E_NONFINITE and keeps running must keep getting status codes, never a
     CUDA fault: the cell grid of a structure with a bead at 1e30 A (or NaN) once overflowed its integer arithmetic."""
@@ -509,7 +527,7 @@ def test_a_blown_up_structure_reports_errors_but_stays_memory_safe(var):
 
 # ---------------------------------------------------------------------------------------------- NEXT-2: Hybrid Taus
 @pytest.mark.parametrize("var", [dict(mode=1, lanes_per_bead=4), dict(mode=2), dict(mode=0), dict(mode=1, reorder=1),
-                                 dict(mode=3), dict(mode=3, chunk_beads=60), dict(mode=3, chunk_beads=60, lanes_per_bead=4)], ids=str)
+                                 dict(mode=3), dict(mode=3, chunk_beads=60), dict(mode=3, chunk_beads=60, resident_variant=2)], ids=str)
 def test_hybrid_taus_noise_matches_the_oracle(var):
     """params.rng = 1: the paper's per-bead Hybrid Taus generator (Alg. 6).  Same seeds, same state stream per bead on
     both sides -> coordinates within 1e-3 A after 100 steps; fixed beads draw nothing; run splits do not matter."""
@@ -563,3 +581,109 @@ def test_mode3_native_table_in_global_memory(var):
     assert np.array_equal(a.get_coords(), b.get_coords())
     o = sopo.from_workload(w); o.run(130)
     assert np.abs(b.get_coords() - o.get_coords()).max() <= 2e-3
+
+
+# ---------------------------------------------------------------------------------------------- NEXT-1: series at a stride
+def _series_case(w, p, T, var, n_steps, stride):
+    """The series recorded inside ONE sop_run equals (i) what the on-demand getters return when the same run is split by
+    hand at every sample (bit for bit: the same kernels on the same coordinates) and (ii) the oracle's observables and
+    energies at the GPU's coordinates of every sample (the 2e-5 / 1e-5 bars of the getters)."""
+    m = sop()
+    a = m.Sop(w.xyz, w.bonds, w.native, dict(p, obs_stride=stride, obs_capacity=n_steps // stride), n_traj=T, **var)
+    a.run(n_steps)
+    steps, ser = a.get_observable_series()
+    assert steps.tolist() == list(range(stride, n_steps + 1, stride)) and ser.shape == (len(steps), T, 10)
+    b = m.Sop(w.xyz, w.bonds, w.native, p, n_traj=T, **var)
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, p, n_traj=T, list_builder=1 if w.n_beads > 5000 else 0)
+    for q, st in enumerate(steps):
+        b.run(stride)
+        assert np.array_equal(b.get_observables(), ser[q, :, :4]) and np.array_equal(b.get_energies(), ser[q, :, 4:])
+        if q % max(1, len(steps) // 8) == 0 or q == len(steps) - 1:
+            x = b.get_coords()
+            o.set_coords(x.astype(np.float64)); o.step = int(st)
+            ref = o.get_observables()
+            scale = np.abs(ref) + 1e-3
+            assert (np.abs(ser[q, :, :4] - ref) <= 2e-5 * scale + 1e-6).all(), (st, ser[q, :, :4], ref)
+            check_energies(ser[q, :, 4:], o.get_energies())
+    assert np.array_equal(a.get_coords(), b.get_coords())       # recording does not change the trajectory
+    return steps, ser
+
+
+@pytest.mark.parametrize("var", [dict(mode=1), dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=24, R_pl=20.0),
+                                 dict(mode=3, chunk_beads=24, R_pl=20.0, resident_variant=2)], ids=str)
+def test_observable_series_small(var):
+    var = dict(var)
+    w = gen.tiny(64, 8)
+    zmax = float(w.xyz[:, 2].max())
+    p = dict(w.params, fixed=[0, 5], pulled=[63, 20], pull_k=0.05, pull_v=1e-3, pull_dir=[0.6, 0.0, 0.8],
+             tip_on=1, tip_R=50.0, tip_eps=1.0, tip_sigma=3.8, tip_c0=[0.0, 0.0, zmax + 53.0],
+             tip_dir=[0.0, 0.0, -1.0], tip_v=1e-3)
+    if "R_pl" in var:
+        p = dict(p, R_pl=var.pop("R_pl"), pl_interval=100)
+    steps, ser = _series_case(w, p, 3, var, 300, 10)
+    # ring semantics: a capacity of 4 keeps the last four samples; stride 0 stops the recording
+    c = sop().Sop(w.xyz, w.bonds, w.native, dict(p, obs_stride=10, obs_capacity=4), n_traj=3, **var)
+    c.run(300)
+    st4, s4 = c.get_observable_series()
+    assert st4.tolist() == [270, 280, 290, 300] and np.array_equal(s4, ser[-4:])
+    c.set_observable_stride(0); c.run(50)
+    assert c.get_observable_series()[0].tolist() == [270, 280, 290, 300]
+
+
+@pytest.mark.parametrize("k", [2, 3])
+def test_observable_series_full_configs(k):
+    """f(R) of the pulled fiber (X, cantilever force) and the force-indentation curve of the shell (tip force
+    against the advance) at stride 10 over 1000 steps of one sop_run."""
+    w = gen.make_config(k)
+    steps, ser = _series_case(w, w.params, 1, {}, 1000, 10)
+    if k == 2:
+        f = ser[:, 0, 2]
+        # r_f t = kappa v t (PAPER.md:259) plus kappa times the thermal excursion of the pulled bead (a few tenths of an A)
+        assert np.polyfit(steps.astype(float), f, 1)[0] > 0 and abs(f[-1] - 0.05 * 1e-3 * 1000) < 0.1
+        assert ser[:, 0, 1].min() > 5000.0
+    else:
+        assert (ser[:, 0, 3] > 0).all() and ser[-1, 0, 3] > ser[0, 0, 3]           # the tip advances: the shell pushes back harder
+
+
+# ---------------------------------------------------------------------------------------------- exchange protocol under skew
+@pytest.mark.parametrize("variant", [1, 2])
+def test_mode3_exchange_is_exact_when_a_chunk_runs_late(variant):
+    """SOP_TEST_SKEW makes one chunk sleep before it publishes on chosen steps (filter steps and the steps around them):
+    its neighbours then run up to the limits the protocol allows.  10^4 steps must be bit-identical to the unskewed run,
+    on a small chunked system and on the 148-chunk shell; no wait may time out."""
+    cases = [(gen.two_chains(150, 3, R_pl=20.0), dict(mode=3, chunk_beads=30, resident_variant=variant), 10000, "2,3,50000"),
+             (gen.make_config(3), dict(mode=3, resident_variant=variant), 2000, "70,7,50000")]
+    for w, var, n, skew in cases:
+        a = sop().from_workload(w, **var); a.run(n); xa = a.get_coords(); a.close()
+        os.environ["SOP_TEST_SKEW"] = skew
+        try:
+            b = sop().from_workload(w, **var); b.run(n); xb = b.get_coords(); b.close()
+        finally:
+            del os.environ["SOP_TEST_SKEW"]
+        assert np.array_equal(xa, xb), (w.name, skew)
+
+
+# ---------------------------------------------------------------------------------------------- P11: long-run ensemble
+def test_p11_long_run_ensemble_means_different_seeds():
+    """SURVEY P11 / north_star: GPU and oracle with DIFFERENT seeds on a config-0-like chain (N = 128), 64 trajectories each,
+    10^5 steps of which the first 10^4 are discarded; the per-trajectory time averages of the total energy and of Rg
+    (sampled every 100 steps; on the GPU through the series recorded inside sop_run) are the independent samples:
+    |m_gpu - m_cpu| <= 3 sqrt(SE_gpu^2 + SE_cpu^2)."""
+    w = gen.config0()
+    T, n, burn, stride = 64, 100000, 10000, 100
+    s = sop().Sop(w.xyz, w.bonds, w.native, dict(w.params, seed=0xA11CE, obs_stride=stride, obs_capacity=n // stride), n_traj=T)
+    s.run(n)
+    steps, ser = s.get_observable_series()
+    keep = steps > burn
+    g_e, g_rg = ser[keep, :, 9].mean(axis=0), ser[keep, :, 0].mean(axis=0)
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, dict(w.params, seed=0xB0B), n_traj=T)
+    o.run(burn)
+    acc_e, acc_rg, cnt = np.zeros(T), np.zeros(T), 0
+    for _ in range((n - burn) // stride):
+        o.run(stride)
+        acc_e += o.get_energies()[:, 5]; acc_rg += o.get_observables()[:, 0]; cnt += 1
+    c_e, c_rg = acc_e / cnt, acc_rg / cnt
+    for name, g, c in (("energy", g_e, c_e), ("Rg", g_rg, c_rg)):
+        se = math.sqrt(g.var(ddof=1) / T + c.var(ddof=1) / T)
+        assert abs(g.mean() - c.mean()) <= 3 * se, (name, g.mean(), c.mean(), se)
+        assert se < 0.02 * abs(c.mean())                      # the test has resolving power: 3 SE is a few per cent at most
