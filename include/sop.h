@@ -61,6 +61,11 @@ typedef struct {
   int32_t cap_nb, cap_pl;            /* row capacities (the paper's M); 0 -> chosen from the native
                                         structure (max count within the cutoff * 1.15 + 8) */
   float dt_over_zeta, kT;            /* h/xi and k_B T of Alg. 7 line 5 */
+  const float *kT_per_traj;          /* HOST [n_traj] or NULL -> kT for all: one temperature per run of a many-runs batch (NEXT-4;
+                                        PAPER.md:310, parallel tempering / Replica Exchange); see sop_replica_exchange */
+  int32_t integrator;                /* 0 / 1 first order, Alg. 7 line 5; 2 second order: the predictor-corrector whose
+                                        mean recursion is Eq. (5) (reading R14): two force evaluations per
+                                        step, mode 1 and rng = 0 only */
   uint64_t seed;                     /* Philox4x32-10 key = (seed lo, seed hi) */
   int32_t traj_offset;               /* global index of local trajectory 0; goes into Philox counter word 1 so
                                         that a batch sharded over GPUs reproduces the unsharded batch */
@@ -133,6 +138,14 @@ int sop_get_observables(sop_handle *, double *o_out /*HOST [T][4]*/);
  * (may be NULL).  Synchronises.  sop_set_observable_stride changes the stride (0 = stop recording). */
 int sop_set_observable_stride(sop_handle *, int32_t stride);
 int sop_get_observable_series(sop_handle *, double *o_out, int64_t *steps_out, int32_t max_samples, int32_t *n_out);
+/* NEXT-4: one sweep of replica exchange over the batch.  For every pair of trajectories (t, t+1) with
+ * t = parity (mod 2), swap their TEMPERATURES with the Metropolis probability min(1, exp((1/kT_t - 1/kT_t+1)(E_t - E_t+1))),
+ * E = total potential energy at the current coordinates (the device-side reduction of sop_get_energies, decided in fp64);
+ * the uniform of pair t is the first word of Philox4x32-10(counter = (traj_offset + t, 'REX!', sweep lo, sweep hi), key = seed)
+ * mapped to (0, 1].  accepted_out: HOST [n_traj / 2] flags of the pairs tried (index t / 2), may be NULL.  Needs
+ * params.kT_per_traj.  sop_get_temperatures: HOST [n_traj] current kT of every trajectory. */
+int sop_replica_exchange(sop_handle *, int32_t parity, uint64_t sweep, int32_t *accepted_out);
+int sop_get_temperatures(sop_handle *, float *kT_out);
 /* Deterministic force (no noise) at the current coordinates with the current L2, incl. external terms. */
 int sop_get_forces(sop_handle *, float *f_out /*HOST [T][N][3]*/);
 /* Row counts and rows (ascending caller index j, padded with -1 to cap) of trajectory traj.

@@ -30,6 +30,7 @@ struct sopo_handle {
   sopo_params p;
   unsigned char *is_fixed;        /* [N] */
   uint32_t *taus;                 /* [T][N][4] Hybrid Taus states (params.rng == 1) */
+  double *kT_t;                   /* [T] temperature of every run */
   int32_t *pulled;                /* [n_pulled] */
   double *native;                 /* [N][3] promoted native coordinates (anchors of the pulled beads) */
   int64_t *excl_ptr; int32_t *excl_idx;   /* bonded + native partners of each bead, ascending */
@@ -267,6 +268,9 @@ int sopo_create(const sopo_topology *tp, const float *native_xyz, const sopo_par
   h->p.fixed = NULL; h->p.pulled = h->pulled;
 
   h->r = (double *)malloc(sizeof(double) * 3 * (size_t)N * (size_t)n_traj);
+  h->kT_t = (double *)malloc(sizeof(double) * (size_t)n_traj);
+  for (int32_t t = 0; t < n_traj; ++t) h->kT_t[t] = p->kT_per_traj ? p->kT_per_traj[t] : p->kT;
+  h->p.kT_per_traj = NULL;
   h->taus = NULL;
   if (p->rng == 1) {
     h->taus = (uint32_t *)malloc(sizeof(uint32_t) * 4 * (size_t)N * (size_t)n_traj);
@@ -292,7 +296,7 @@ void sopo_destroy(sopo_handle *h) {
   if (!h) return;
   free(h->bond_i); free(h->bond_j); free(h->bond_r0);
   free(h->nat_i); free(h->nat_j); free(h->nat_r0); free(h->nat_eps);
-  free(h->taus); free(h->is_fixed); free(h->pulled); free(h->native); free(h->excl_ptr); free(h->excl_idx); free(h->r);
+  free(h->taus); free(h->kT_t); free(h->is_fixed); free(h->pulled); free(h->native); free(h->excl_ptr); free(h->excl_idx); free(h->r);
   if (h->L1) for (int32_t t = 0; t < h->T; ++t) csr_free(&h->L1[t]);
   if (h->L2) for (int32_t t = 0; t < h->T; ++t) csr_free(&h->L2[t]);
   free(h->L1); free(h->L2);
@@ -563,7 +567,36 @@ static int step_one(sopo_handle *h, int32_t t, int64_t step, double *fbuf) {
   double *r = h->r + 3 * (size_t)N * (size_t)t;
   int status = eval(h, r, &h->L2[t], step, NULL, fbuf);
   const double D = h->p.dt_over_zeta;
-  const double amp = sqrt(2.0 * h->p.kT * D);
+  const double amp = sqrt(2.0 * h->kT_t[t] * D);
+  if (h->p.integrator == 2) {
+    /* Second order (reading R14).  Eq. (5) is the mean recursion of the predictor-corrector
+     *   r' = r + f(r, t_n) h/xi + G,   r(t_n + h) = r + (h / 2 xi) [f(r, t_n) + f(r', t_n)] + G
+     * (for the paper's f = r_f t_n - K_sp X:  X + (r_f t_n/xi - X/tau) h + (X/(2 tau^2) - r_f t_n/(2 tau xi)) h^2), with the
+     * same random displacement G = g sqrt(2 kT h/xi) in both stages and the lists, the pulling spring and the indenter at
+     * t_n in both force evaluations. */
+    double *rp = (double *)malloc(sizeof(double) * 3 * (size_t)N), *gs = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double *f2 = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    for (int32_t i = 0; i < N; ++i) {
+      double g[3] = { 0, 0, 0 };
+      if (!h->is_fixed[i]) sopo_normals(h->p.seed, (uint32_t)i, (uint32_t)(h->p.traj_offset + t), (uint64_t)step, g);
+      for (int a = 0; a < 3; ++a) {
+        gs[3 * (size_t)i + a] = g[a];
+        rp[3 * (size_t)i + a] = h->is_fixed[i] ? r[3 * (size_t)i + a] : r[3 * (size_t)i + a] + D * fbuf[3 * (size_t)i + a] + amp * g[a];
+      }
+    }
+    int rc = eval(h, rp, &h->L2[t], step, NULL, f2);
+    if (rc && !status) status = rc;
+    for (int32_t i = 0; i < N; ++i) {
+      if (h->is_fixed[i]) continue;
+      for (int a = 0; a < 3; ++a) {
+        double v = r[3 * (size_t)i + a] + 0.5 * D * (fbuf[3 * (size_t)i + a] + f2[3 * (size_t)i + a]) + amp * gs[3 * (size_t)i + a];
+        if (!isfinite(v)) status = status ? status : SOPO_E_NONFINITE;
+        r[3 * (size_t)i + a] = v;
+      }
+    }
+    free(rp); free(gs); free(f2);
+    return status;
+  }
   for (int32_t i = 0; i < N; ++i) {
     if (h->is_fixed[i]) continue;
     double g[3];
@@ -576,6 +609,46 @@ static int step_one(sopo_handle *h, int32_t t, int64_t step, double *fbuf) {
     }
   }
   return status;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-4: replica exchange (the many-runs-per-GPU approach "in conjunction with parallel tempering
+ * algorithms, including variants of the Replica Exchange Method").  Two runs at inverse temperatures b_i, b_j and
+ * potential energies E_i, E_j swap temperatures with the Metropolis probability min(1, exp((b_i - b_j)(E_i - E_j))):
+ * the ratio of the Boltzmann weights of the swapped and the unswapped pair, exp(-b_i E_j - b_j E_i) / exp(-b_i E_i - b_j E_j).
+ * ------------------------------------------------------------------------------------------------ */
+double sopo_rex_probability(double E_i, double E_j, double kT_i, double kT_j) {
+  double d = (1.0 / kT_i - 1.0 / kT_j) * (E_i - E_j);
+  return d >= 0.0 ? 1.0 : exp(d);
+}
+int sopo_rex_accept(double E_i, double E_j, double kT_i, double kT_j, double u) {
+  return u <= sopo_rex_probability(E_i, E_j, kT_i, kT_j) ? 1 : 0;      /* u in (0, 1]: probability 1 always accepts */
+}
+
+int sopo_replica_exchange(sopo_handle *h, int32_t parity, uint64_t sweep, int32_t *accepted) {
+  if (!h || (parity != 0 && parity != 1)) return SOPO_E_ARG;
+  int status = SOPO_OK;
+  for (int32_t t = parity; t + 1 < h->T; t += 2) {
+    double e_i[6], e_j[6];
+    int rc = eval(h, h->r + 3 * (size_t)h->N * (size_t)t, &h->L2[t], h->step, e_i, NULL);
+    if (rc && !status) status = rc;
+    rc = eval(h, h->r + 3 * (size_t)h->N * (size_t)(t + 1), &h->L2[t + 1], h->step, e_j, NULL);
+    if (rc && !status) status = rc;
+    uint32_t ctr[4] = { (uint32_t)(h->p.traj_offset + t), 0x52455821u, (uint32_t)(sweep & 0xFFFFFFFFu), (uint32_t)(sweep >> 32) };
+    uint32_t key[2] = { (uint32_t)(h->p.seed & 0xFFFFFFFFu), (uint32_t)(h->p.seed >> 32) }, x[4];
+    sopo_philox4x32_10(ctr, key, x);
+    double u = ((double)(x[0] >> 8) + 1.0) * (1.0 / 16777216.0);
+    int acc = sopo_rex_accept(e_i[5], e_j[5], h->kT_t[t], h->kT_t[t + 1], u);
+    if (acc) { double tmp = h->kT_t[t]; h->kT_t[t] = h->kT_t[t + 1]; h->kT_t[t + 1] = tmp; }
+    if (accepted) accepted[t / 2] = acc;
+  }
+  return status;
+}
+
+int sopo_get_temperatures(sopo_handle *h, double *kT_out) {
+  if (!h || !kT_out) return SOPO_E_ARG;
+  memcpy(kT_out, h->kT_t, sizeof(double) * (size_t)h->T);
+  return SOPO_OK;
 }
 
 /* Schedule: after the update that makes step = s, if s % pl_interval == 0 the

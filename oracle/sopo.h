@@ -47,6 +47,10 @@ typedef struct {
                                                   cell list (tests prove it equal to 0; used for big N only) */
   int32_t rng;                                 /* 0 counter-based Philox (reading R6); 1 the paper's Hybrid Taus
                                                   (Alg. 6), state per bead, reading R12 */
+  int32_t integrator;                          /* 0/1 first order, Alg. 7 line 5; 2 second order: the scheme whose
+                                                  mean recursion is Eq. (5) (reading R14) */
+  const double *kT_per_traj;                   /* [n_traj] or NULL -> kT for all: one temperature per run of a many-runs batch
+                                                  ("parallel tempering ... Replica Exchange") */
 } sopo_params;
 
 enum { SOPO_OK = 0, SOPO_E_ARG = -1, SOPO_E_CAP = -3, SOPO_E_FENE = -4, SOPO_E_NONFINITE = -5 };
@@ -85,6 +89,17 @@ void sopo_normals_batch(uint64_t seed, uint32_t bead0, uint32_t n_beads, uint32_
                          double *g_out /*[n_beads][3]*/);
 int  sopo_pred(const double a[3], const double b[3], double R);        /* the canonical fp32 list predicate */
 int  sopo_num_threads(void);
+
+/* NEXT-4: replica exchange over the batch.  One sweep: for every pair (t, t+1) with t = parity (mod 2), swap
+ * the TEMPERATURES of the two runs with the Metropolis probability min(1, exp((1/kT_t - 1/kT_t+1)(E_t - E_t+1))), E = total
+ * potential energy of the run at its current coordinates; the uniform of pair t in sweep `sweep` is the first word of
+ * Philox4x32-10(counter = (t, 'REX!', sweep lo, sweep hi), key = seed) mapped to (0, 1] like u_a of sopo_normals.
+ * accepted (may be NULL): [n_traj / 2] flags of the pairs tried (pair index t / 2). */
+int  sopo_replica_exchange(sopo_handle *, int32_t parity, uint64_t sweep, int32_t *accepted);
+int  sopo_get_temperatures(sopo_handle *, double *kT_out /*[n_traj]*/);
+/* the acceptance probability and the decision, exposed for the pins */
+double sopo_rex_probability(double E_i, double E_j, double kT_i, double kT_j);
+int  sopo_rex_accept(double E_i, double E_j, double kT_i, double kT_j, double u);
 
 #ifdef __cplusplus
 }

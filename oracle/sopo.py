@@ -34,7 +34,7 @@ class _Params(C.Structure):
                 ("pull_k", C.c_double), ("pull_v", C.c_double), ("pull_dir", C.c_double * 3),
                 ("tip_on", C.c_int32), ("tip_R", C.c_double), ("tip_eps", C.c_double), ("tip_sigma", C.c_double),
                 ("tip_c0", C.c_double * 3), ("tip_dir", C.c_double * 3), ("tip_v", C.c_double),
-                ("list_builder", C.c_int32), ("rng", C.c_int32)]
+                ("list_builder", C.c_int32), ("rng", C.c_int32), ("integrator", C.c_int32), ("kT_per_traj", C.c_void_p)]
 
 
 def lib():
@@ -68,6 +68,11 @@ def lib():
         L.sopo_normals_batch.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, C.c_void_p]
         L.sopo_normals_batch.restype = None
         L.sopo_pred.argtypes = [C.c_void_p, C.c_void_p, C.c_double]
+        L.sopo_replica_exchange.argtypes = [C.c_void_p, C.c_int32, C.c_uint64, C.c_void_p]
+        L.sopo_get_temperatures.argtypes = [C.c_void_p, C.c_void_p]
+        L.sopo_rex_probability.argtypes = [C.c_double] * 4
+        L.sopo_rex_probability.restype = C.c_double
+        L.sopo_rex_accept.argtypes = [C.c_double] * 5
         _lib = L
     return _lib
 
@@ -142,6 +147,9 @@ class Oracle:
         pp.tip_v = f32(p.get("tip_v", 0.0))
         pp.list_builder = int(list_builder)
         pp.rng = int(p.get("rng", 0))
+        pp.integrator = int(p.get("integrator", 0))
+        self._kT_t = None if p.get("kT_per_traj") is None else np.ascontiguousarray([f32(v) for v in p["kT_per_traj"]], np.float64)
+        pp.kT_per_traj = None if self._kT_t is None else self._kT_t.ctypes.data
         self._h = C.c_void_p()
         rc = L.sopo_create(C.byref(tp), self._xyz.ctypes.data, C.byref(pp), self.T, C.byref(self._h))
         if rc:
@@ -187,6 +195,17 @@ class Oracle:
         """[T][4]: Rg, end-to-end distance X, cantilever force, tip force."""
         out = np.zeros((self.T, 4), np.float64)
         self._chk(lib().sopo_get_observables(self._h, out.ctypes.data), "get_observables")
+        return out
+
+    def replica_exchange(self, parity, sweep):
+        """one sweep of temperature swaps between runs (t, t+1), t = parity mod 2 -> accepted[T // 2] (pairs tried)"""
+        acc = np.zeros(max(1, self.T // 2), np.int32)
+        self._chk(lib().sopo_replica_exchange(self._h, int(parity), int(sweep), acc.ctypes.data), "replica_exchange")
+        return acc
+
+    def get_temperatures(self):
+        out = np.zeros(self.T, np.float64)
+        self._chk(lib().sopo_get_temperatures(self._h, out.ctypes.data), "get_temperatures")
         return out
 
     def get_forces(self):
@@ -236,6 +255,14 @@ class Oracle:
 
 def from_workload(w, n_traj=None, **kw):
     return Oracle(w.xyz, w.bonds, w.native, w.params, n_traj=w.n_traj if n_traj is None else n_traj, **kw)
+
+
+def rex_probability(E_i, E_j, kT_i, kT_j):
+    return float(lib().sopo_rex_probability(float(E_i), float(E_j), float(kT_i), float(kT_j)))
+
+
+def rex_accept(E_i, E_j, kT_i, kT_j, u):
+    return bool(lib().sopo_rex_accept(float(E_i), float(E_j), float(kT_i), float(kT_j), float(u)))
 
 
 def taus_step(y):

@@ -34,7 +34,7 @@ struct Plan {                     // everything that depends only on (topology, 
   // workspace offsets
   size_t off_pos0, off_pos1, off_carry, off_force, off_bond, off_natptr, off_nattab, off_nateps, off_exclptr,
       off_exclidx, off_adotn, off_plcnt, off_plidx, off_nbcnt, off_nbidx, off_bbox, off_grid, off_cellof,
-      off_cellcnt, off_cellstart, off_cellbead, off_cellpos, off_taus, off_flags, off_epart, off_eout, off_bar, off_series, total;
+      off_cellcnt, off_cellstart, off_cellbead, off_cellpos, off_taus, off_flags, off_epart, off_eout, off_bar, off_series, off_kTt, off_ampt, off_rexacc, total;
   // mode 3 (SM-resident kernel): chunking, launch shape, shared-memory carve-up, workspace
   bool res_ok = false;
   std::string res_why;
@@ -455,11 +455,17 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.block = p->block_size > 0 ? p->block_size : 256;
   if (pl.block % 32 || pl.block > 1024) return fail(SOP_E_ARG, "block_size must be a multiple of 32, <= 1024");
   if (p->mode < 0 || p->mode > 3) return fail(SOP_E_ARG, "mode must be 0, 1, 2 or 3");
+  if (p->integrator < 0 || p->integrator > 2) return fail(SOP_E_ARG, "integrator must be 0, 1 or 2");
+  if (p->integrator == 2 && (p->rng != 0 || p->mode > 1))
+    return fail(SOP_E_ARG, "integrator = 2 (second order, Eq. (5)) runs in mode 1 with rng = 0");
+  if (p->kT_per_traj)
+    for (int t = 0; t < T; ++t)
+      if (!(p->kT_per_traj[t] >= 0)) return fail(SOP_E_ARG, "bad kT_per_traj");
   if (p->obs_stride < 0 || p->obs_capacity < 0 || (p->obs_stride > 0 && p->obs_capacity < 1))
     return fail(SOP_E_ARG, "obs_stride needs obs_capacity >= 1");
   if (p->resident_variant < 0 || p->resident_variant > 2) return fail(SOP_E_ARG, "resident_variant must be 0, 1 or 2");
   if (p->rng != 0 && p->rng != 1) return fail(SOP_E_ARG, "rng must be 0 (Philox) or 1 (Hybrid Taus)");
-  pl.mode = p->mode;
+  pl.mode = p->integrator == 2 ? 1 : p->mode;
   if (pl.mode == 0 || pl.mode == 3) {
     plan_resident(tp, p, x, pl);
     if (pl.mode == 3 && !pl.res_ok) return fail(SOP_E_ARG, "mode 3 is not possible here: " + pl.res_why);
@@ -497,6 +503,9 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.off_eout = take((size_t)T * 6 * 8);
   pl.off_bar = take(256);
   pl.off_series = take(p->obs_capacity > 0 ? (size_t)p->obs_capacity * T * 10 * 8 : 0);
+  pl.off_kTt = take(p->kT_per_traj ? (size_t)T * 4 : 0);
+  pl.off_ampt = take(p->kT_per_traj ? (size_t)T * 4 : 0);
+  pl.off_rexacc = take(p->kT_per_traj ? (size_t)T * 4 : 0);
   if (pl.mode == 3) {
     const ResDev &R = pl.R;
     const bool multi = R.C > 1;
@@ -555,6 +564,28 @@ void launch_step(sop_handle *h, bool forces) {
     case 8: launch_step_g<8>(h, forces); break;
     case 16: launch_step_g<16>(h, forces); break;
     default: launch_step_g<32>(h, forces); break;
+  }
+}
+
+template <int G>
+void launch_step2_g(sop_handle *h, int stage) {
+  const SysDev &S = h->S;
+  const long long threads = (long long)S.n_inst * G;
+  const int block = h->plan.block;
+  const unsigned grid = (unsigned)((threads + block - 1) / block);
+  if (h->plan.comp) k_step2<G, true><<<grid, block, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, stage);
+  else k_step2<G, false><<<grid, block, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, stage);
+  h->launches++;
+}
+
+void launch_step2(sop_handle *h, int stage) {
+  switch (h->plan.lanes) {
+    case 1: launch_step2_g<1>(h, stage); break;
+    case 2: launch_step2_g<2>(h, stage); break;
+    case 4: launch_step2_g<4>(h, stage); break;
+    case 8: launch_step2_g<8>(h, stage); break;
+    case 16: launch_step2_g<16>(h, stage); break;
+    default: launch_step2_g<32>(h, stage); break;
   }
 }
 
@@ -823,7 +854,7 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
   }
   const int N = pl.N, T = pl.T;
   h->prm = *p;
-  h->prm.fixed = nullptr; h->prm.pulled = nullptr;
+  h->prm.fixed = nullptr; h->prm.pulled = nullptr; h->prm.kT_per_traj = nullptr;
   h->stream = (cudaStream_t)p->stream;
   h->ws = (char *)d_workspace;
 
@@ -938,6 +969,7 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
   S.tip_cx = p->tip_c0[0]; S.tip_cy = p->tip_c0[1]; S.tip_cz = p->tip_c0[2];
   S.tip_nx = p->tip_dir[0]; S.tip_ny = p->tip_dir[1]; S.tip_nz = p->tip_dir[2];
   S.taus = p->rng == 1 ? (uint4 *)(w + pl.off_taus) : nullptr;
+  S.amp_t = p->kT_per_traj ? (const float *)(w + pl.off_ampt) : nullptr;
   S.flags = (int *)(w + pl.off_flags);
 
   // ---- upload (synchronous copies from pageable host vectors; create is not on the hot path)
@@ -960,6 +992,11 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
   acc(up(pl.off_exclptr, excl_ptr.data(), excl_ptr.size() * 4));
   acc(up(pl.off_exclidx, excl_idx.data(), excl_idx.size() * 4));
   if (p->n_pulled > 0) acc(up(pl.off_adotn, adotn.data(), adotn.size() * 4));
+  std::vector<float> kT_t, amp_t;
+  if (p->kT_per_traj) {
+    for (int t = 0; t < T; ++t) { kT_t.push_back(p->kT_per_traj[t]); amp_t.push_back((float)std::sqrt(2.0 * (double)p->kT_per_traj[t] * (double)p->dt_over_zeta)); }
+    acc(up(pl.off_kTt, kT_t.data(), (size_t)T * 4)); acc(up(pl.off_ampt, amp_t.data(), (size_t)T * 4));
+  }
   acc(cudaStreamSynchronize(st));
   if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); delete h; return fail(SOP_E_CUDA, "upload: " + m); }
 
@@ -1055,8 +1092,8 @@ int sop_run(sop_handle *h, int64_t n_steps) {
       if (sample_due) { rc = record_sample(h); if (rc) return rc; }
     } else {
       span_begin(h, SPAN_STEP, 1);
-      launch_step(h, false);
-      h->cur ^= 1; h->step++; left--;
+      if (h->prm.integrator == 2) { launch_step2(h, 0); launch_step2(h, 1); h->step++; left--; }     // (the result is back in layer cur)
+      else { launch_step(h, false); h->cur ^= 1; h->step++; left--; }
       if (!h->S.static_l1 && h->step % plv == 0) { int rc = launch_build_l1(h); if (rc) return rc; }
       if (h->step % nb == 0) launch_filter(h);
       if (ost > 0 && h->step % ost == 0) { int rc = record_sample(h); if (rc) return rc; }
@@ -1170,6 +1207,42 @@ int sop_get_energies(sop_handle *h, double *e_out) {
     e[5] = e[0] + e[1] + e[2] + e[3] + e[4];
   }
   return rc;
+}
+
+int sop_replica_exchange(sop_handle *h, int32_t parity, uint64_t sweep, int32_t *accepted_out) {
+  if (!h || (parity != 0 && parity != 1)) return fail(SOP_E_ARG, "bad argument", h);
+  if (!h->S.amp_t) return fail(SOP_E_ARG, "replica exchange needs params.kT_per_traj", h);
+  const SysDev &S = h->S;
+  double *partial = (double *)(h->ws + h->plan.off_epart), *d_e = (double *)(h->ws + h->plan.off_eout);
+  int *d_acc = (int *)(h->ws + h->plan.off_rexacc);
+  dim3 grid((unsigned)h->plan.energy_blocks, (unsigned)S.T);
+  k_energy<<<grid, 256, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, partial);
+  k_energy_final<<<(S.T * 5 + 127) / 128, 128, 0, h->stream>>>(S.T, h->plan.energy_blocks, partial, d_e, 6);
+  const int pairs = (S.T + 1) / 2;
+  k_replica_exchange<<<(pairs + 127) / 128, 128, 0, h->stream>>>(S, d_e, (float *)(h->ws + h->plan.off_kTt), (float *)(h->ws + h->plan.off_ampt),
+                                                                parity, (unsigned long long)sweep, d_acc);
+  h->launches += 3;
+  int rc = check_launch(h, "replica exchange");
+  if (rc) return rc;
+  if (accepted_out) {
+    const int tried = (S.T - parity) / 2;
+    for (int q = 0; q < S.T / 2; ++q) accepted_out[q] = 0;
+    if (tried > 0) {
+      std::vector<int> tmp((size_t)S.T, 0);
+      CUDA_OK(cudaMemcpyAsync(tmp.data(), d_acc, (size_t)S.T * 4, cudaMemcpyDeviceToHost, h->stream));
+      rc = read_flags(h);
+      for (int t = parity; t + 1 < S.T; t += 2) accepted_out[t / 2] = tmp[t / 2];
+      return rc;
+    }
+  }
+  return SOP_OK;
+}
+
+int sop_get_temperatures(sop_handle *h, float *kT_out) {
+  if (!h || !kT_out) return fail(SOP_E_ARG, "null argument", h);
+  if (!h->S.amp_t) { for (int t = 0; t < h->S.T; ++t) kT_out[t] = h->prm.kT; return SOP_OK; }
+  CUDA_OK(cudaMemcpyAsync(kT_out, h->ws + h->plan.off_kTt, (size_t)h->S.T * 4, cudaMemcpyDeviceToHost, h->stream));
+  return read_flags(h);
 }
 
 int sop_get_observables(sop_handle *h, double *o_out) {

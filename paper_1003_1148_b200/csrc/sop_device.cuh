@@ -60,6 +60,7 @@ struct SysDev {
   float c_rep_e;                    // eps_r sigma^6
   float R_nb2, R_pl2;               // (float)(R*R): the canonical cutoffs of the list predicate
   float D, amp;                     // h/xi and sqrt(2 kT h/xi)
+  const float *amp_t;               // [T] sqrt(2 kT_t h/xi): one temperature per trajectory (NEXT-4), or nullptr
   uint32_t seed_lo, seed_hi;
   int traj_offset;
   int has_pull; float pull_k, pull_v, pull_nx, pull_ny, pull_nz;
@@ -278,10 +279,12 @@ __device__ __forceinline__ float3 gaussian3_taus(uint4 *state) {
 }
 
 // a9: the position update of Alg. 7 line 5 given the three normals, optionally Kahan-compensated (R10).
+__device__ __forceinline__ float amp_of(const SysDev &S, int t) { return S.amp_t ? __ldg(S.amp_t + t) : S.amp; }
+
 template <bool COMP>
 __device__ __forceinline__ float4 langevin_apply(const SysDev &S, const float4 &ri, const float3 &gn, float fx, float fy,
-                                                 float fz, float4 *carry_slot, int &flag) {
-  float dx = S.D * fx + S.amp * gn.x, dy = S.D * fy + S.amp * gn.y, dz = S.D * fz + S.amp * gn.z;
+                                                 float fz, float4 *carry_slot, int &flag, float amp) {
+  float dx = S.D * fx + amp * gn.x, dy = S.D * fy + amp * gn.y, dz = S.D * fz + amp * gn.z;
   float4 out;
   if (COMP) {
     float4 c = *carry_slot;
@@ -306,7 +309,7 @@ __device__ __forceinline__ float4 langevin_update(const SysDev &S, const float4 
                                                   float4 *carry_slot, int &flag, int inst = 0) {
   if (tag & TAG_FIXED) return ri;                                     // fixed beads are copied unchanged
   float3 gn = S.taus ? gaussian3_taus(S.taus + inst) : gaussian3(S, tag & TAG_ID_MASK, (uint32_t)(S.traj_offset + t), step);
-  return langevin_apply<COMP>(S, ri, gn, fx, fy, fz, carry_slot, flag);
+  return langevin_apply<COMP>(S, ri, gn, fx, fy, fz, carry_slot, flag, amp_of(S, t));
 }
 
 // ------------------------------------------------------------------------------------------------

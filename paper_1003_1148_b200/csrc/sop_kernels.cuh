@@ -33,6 +33,70 @@ __global__ void __launch_bounds__(1024) k_step(SysDev S, int cur, unsigned long 
   if (flag) atomicOr(S.flags, flag);
 }
 
+// ------------------------------------------------------------------------------------------------
+// NEXT-4: the second-order update whose mean recursion is Eq. (5) (reading R14), two launches
+// per step:  stage 0  r' = r + f(r) h/xi + G  -> the other time layer, f(r) -> S.force;
+//            stage 1  r(t + h) = r + (h / 2 xi)[f(r) + f(r')] + G  in place (a thread writes only its own bead of the layer
+//            it reads its own bead from; partners are read from the r' layer).
+// The same Philox draw G in both stages (counter-based: regenerated, never stored); external terms at t_n in both.
+// ------------------------------------------------------------------------------------------------
+template <int G, bool COMP>
+__global__ void __launch_bounds__(1024) k_step2(SysDev S, int cur, unsigned long long step, int stage) {
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int g = (int)(gid / G);
+  const int lane = (int)(gid % G);
+  const bool valid = g < S.n_inst;
+  const int gg = valid ? g : 0;
+  const int t = gg / S.N, i = gg - t * S.N;
+  const float4 *__restrict__ pos_t = S.pos[stage == 0 ? cur : cur ^ 1] + (size_t)t * S.N;
+  const float4 ri = __ldg(pos_t + i);                 // stage 0: r;  stage 1: r'
+  int flag = 0;
+  float3 f = internal_force<G, true>(S, pos_t, i, gg, lane, valid, ri, flag);
+  if (valid && lane == 0) {
+    const uint32_t tag = __float_as_uint(ri.w);
+    external_force(S, i, ri, tag, step, f.x, f.y, f.z, flag);
+    if (!(tag & TAG_FIXED)) {
+      const float3 gn = gaussian3(S, tag & TAG_ID_MASK, (uint32_t)(S.traj_offset + t), step);
+      const float amp = amp_of(S, t);
+      if (stage == 0) {
+        S.force[gg] = make_float4(f.x, f.y, f.z, 0.f);
+        S.pos[cur ^ 1][gg] = langevin_apply<false>(S, ri, gn, f.x, f.y, f.z, nullptr, flag, amp);
+      } else {
+        const float4 f0 = S.force[gg];
+        const float4 r0 = S.pos[cur][gg];
+        S.pos[cur][gg] = langevin_apply<COMP>(S, r0, gn, 0.5f * (f0.x + f.x), 0.5f * (f0.y + f.y), 0.5f * (f0.z + f.z),
+                                              COMP ? S.carry + gg : nullptr, flag, amp);
+      }
+    } else if (stage == 0) {
+      S.pos[cur ^ 1][gg] = ri;
+    }
+  }
+  if (flag) atomicOr(S.flags, flag);
+}
+
+// NEXT-4: one sweep of replica-exchange temperature swaps between trajectories (t, t+1), t = parity mod 2.
+// Metropolis in fp64 on the device-reduced energies: accept if u <= min(1, exp((1/kT_t - 1/kT_t+1)(E_t - E_t+1))), u in (0, 1]
+// from the first word of Philox4x32-10(counter = (global t, 'REX!', sweep lo, sweep hi), key = seed).
+__global__ void k_replica_exchange(SysDev S, const double *e6, float *kT_t, float *amp_t, int parity, unsigned long long sweep, int *accepted) {
+  const int pair = blockIdx.x * blockDim.x + threadIdx.x;
+  const int t = parity + 2 * pair;
+  if (t + 1 >= S.T) return;
+  const double Ei = e6[6 * t] + e6[6 * t + 1] + e6[6 * t + 2] + e6[6 * t + 3] + e6[6 * t + 4];
+  const double Ej = e6[6 * (t + 1)] + e6[6 * (t + 1) + 1] + e6[6 * (t + 1) + 2] + e6[6 * (t + 1) + 3] + e6[6 * (t + 1) + 4];
+  const double d = (1.0 / (double)kT_t[t] - 1.0 / (double)kT_t[t + 1]) * (Ei - Ej);
+  const double prob = d >= 0.0 ? 1.0 : exp(d);
+  const uint4 x = philox4x32_10(make_uint4((uint32_t)(S.traj_offset + t), 0x52455821u, (uint32_t)sweep, (uint32_t)(sweep >> 32)),
+                                make_uint2(S.seed_lo, S.seed_hi));
+  const double u = ((double)(x.x >> 8) + 1.0) * (1.0 / 16777216.0);
+  const int acc = u <= prob ? 1 : 0;
+  if (acc) {
+    const float k0 = kT_t[t], a0 = amp_t[t];
+    kT_t[t] = kT_t[t + 1]; amp_t[t] = amp_t[t + 1];
+    kT_t[t + 1] = k0; amp_t[t + 1] = a0;
+  }
+  if (accepted) accepted[t / 2] = acc;
+}
+
 // initial Hybrid Taus states (Alg. 6 line 1): Philox4x32-10(counter = (bead, traj, 'TAUS', 0), key = seed), with the
 // bits that keep the Tausworthe components off their degenerate states (y1 >= 2, y2 >= 8, y3 >= 16)
 __global__ void k_taus_seed(SysDev S, int cur) {

@@ -296,6 +296,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   unsigned fpar = (unsigned)((step0 / (unsigned long long)nb_interval) & 1ull);      // filter layer of the prologue
   const int cap_b = S.cap_b, cap_nb = S.cap_nb;
   const uint32_t traj = (uint32_t)(S.traj_offset + t);
+  const float amp_tr = amp_of(S, t);
   int flag = 0;
 
   // exclusive scan of n_own 16-bit counts by warp 0 (the caller synchronises)
@@ -751,7 +752,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
         float3 gn;
         if (G > 1) { const float4 g4 = gc[i]; gn = make_float3(g4.x, g4.y, g4.z); }
         else gn = S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step);   // thread per bead already
-        out = langevin_apply<COMP>(S, ri, gn, fx, fy, fz, COMP ? scarry + i : nullptr, flag);
+        out = langevin_apply<COMP>(S, ri, gn, fx, fy, fz, COMP ? scarry + i : nullptr, flag, amp_tr);
       }
       pn[i] = out;
       if (multi) xch_put(xpub + 2 * (inst0 + b0 + i), out, st_n);

@@ -639,7 +639,7 @@ __global__ void __launch_bounds__(1024, 1) k_res2(SysDev S, ResDev R, Res2Dev Q,
     bool vp[P];
     const uint32_t s_own = smem_u32(own), s_halo = smem_u32(halo), s_rows = smem_u32(rows), s_g = smem_u32(sg);
     const uint32_t s_eps = smem_u32(rows_eps), s_ext = smem_u32(sext);
-    const float A = Q.a_ref;
+    const float A = Q.a_ref, amp_tr = amp_of(S, t);
     // one entry of a force row: s = A (1/r^2) (q max(q, 0) - q), q = (par/r^2)^3 (see the header); f_i += s (r_i - r_j)
     auto pair = [&](uint32_t entry, uint32_t base, const float4 &ri, float &fx, float &fy, float &fz) {
       const uint2 en = lds_u2(entry);
@@ -756,7 +756,7 @@ __global__ void __launch_bounds__(1024, 1) k_res2(SysDev S, ResDev R, Res2Dev Q,
             ExtStep ext; ext.vs_pull = e4.x; ext.cx = e4.y; ext.cy = e4.z; ext.cz = e4.w;
             external_force_at(S, b0 + il, r0, tag, ext, ux, uy, uz, flag);
             const float4 g4 = lds_f4(s_g + (uint32_t)((k & 1) * R.chunk + il) * 16u);
-            out = langevin_apply<COMP>(S, r0, make_float3(g4.x, g4.y, g4.z), ux, uy, uz, COMP ? scarry + il : nullptr, flag);
+            out = langevin_apply<COMP>(S, r0, make_float3(g4.x, g4.y, g4.z), ux, uy, uz, COMP ? scarry + il : nullptr, flag, amp_tr);
           }
           sts_f4(s_own + (uint32_t)(((k & 1) ^ 1) * Q.own_stride + il) * 16u, out);
           uint4 *xp = filt ? (fpar ? xf1 : xf0) : (((k + 1) & 1) ? xs1 : xs0);

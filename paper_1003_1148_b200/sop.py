@@ -17,7 +17,7 @@ STATUS = {0: "SOP_OK", -1: "SOP_E_ARG", -2: "SOP_E_CUDA", -3: "SOP_E_LIST_OVERFL
 SYMBOLS = ["sop_query_workspace", "sop_create", "sop_destroy", "sop_run", "sop_sync", "sop_get_coords",
            "sop_set_coords", "sop_get_energies", "sop_get_observables", "sop_get_forces", "sop_get_lists", "sop_get_step", "sop_set_step",
            "sop_device_coords", "sop_get_config", "sop_set_profiling", "sop_get_profile", "sop_last_error",
-           "sop_set_observable_stride", "sop_get_observable_series"]
+           "sop_set_observable_stride", "sop_get_observable_series", "sop_replica_exchange", "sop_get_temperatures"]
 
 
 class _Topology(C.Structure):
@@ -34,6 +34,7 @@ class _Params(C.Structure):
                 ("nb_interval", C.c_int32), ("pl_interval", C.c_int32),
                 ("cap_nb", C.c_int32), ("cap_pl", C.c_int32),
                 ("dt_over_zeta", C.c_float), ("kT", C.c_float),
+                ("kT_per_traj", C.c_void_p), ("integrator", C.c_int32),
                 ("seed", C.c_uint64),
                 ("traj_offset", C.c_int32),
                 ("n_fixed", C.c_int32), ("fixed", C.c_void_p),
@@ -73,6 +74,8 @@ def lib():
         L.sop_get_forces.argtypes = [vp, vp]
         L.sop_get_observables.argtypes = [vp, vp]
         L.sop_set_observable_stride.argtypes = [vp, i32]
+        L.sop_replica_exchange.argtypes = [vp, i32, C.c_uint64, vp]
+        L.sop_get_temperatures.argtypes = [vp, vp]
         L.sop_get_observable_series.argtypes = [vp, vp, vp, i32, C.POINTER(i32)]
         L.sop_get_lists.argtypes = [vp, i32, i32, vp, vp, C.POINTER(i32), C.POINTER(i64)]
         L.sop_get_step.argtypes = [vp, C.POINTER(i64)]
@@ -108,6 +111,7 @@ def _marshal(xyz, bonds, native, params, native_eps, overrides):
     keep["eps"] = None if native_eps is None else np.ascontiguousarray(native_eps, np.float32)
     keep["fixed"] = np.ascontiguousarray(p.get("fixed", []), np.int32)
     keep["pulled"] = np.ascontiguousarray(p.get("pulled", []), np.int32)
+    keep["kT_t"] = None if p.get("kT_per_traj") is None else np.ascontiguousarray(p["kT_per_traj"], np.float32)
     tp = _Topology(len(keep["xyz"]), len(keep["bonds"]), keep["bonds"].ctypes.data, len(keep["native"]),
                    keep["native"].ctypes.data, None if keep["eps"] is None else keep["eps"].ctypes.data)
     pp = _Params()
@@ -119,6 +123,8 @@ def _marshal(xyz, bonds, native, params, native_eps, overrides):
     pp.seed = int(p["seed"]); pp.traj_offset = int(p.get("traj_offset", 0))
     pp.n_fixed = len(keep["fixed"]); pp.fixed = keep["fixed"].ctypes.data
     pp.n_pulled = len(keep["pulled"]); pp.pulled = keep["pulled"].ctypes.data
+    pp.kT_per_traj = None if keep["kT_t"] is None else keep["kT_t"].ctypes.data
+    pp.integrator = int(p.get("integrator", 0))
     pp.pull_k = float(p.get("pull_k", 0.0)); pp.pull_v = float(p.get("pull_v", 0.0))
     pp.pull_dir = (C.c_float * 3)(*[float(v) for v in p.get("pull_dir", [0, 0, 1])])
     pp.tip_on = int(p.get("tip_on", 0))
@@ -201,6 +207,17 @@ class Sop:
         self._chk(lib().sop_get_observables(self._h, out.ctypes.data), "sop_get_observables")
         return out
 
+    def replica_exchange(self, parity, sweep):
+        """one sweep of temperature swaps between trajectories (t, t+1), t = parity mod 2 -> accepted[T // 2]"""
+        acc = np.zeros(max(1, self.T // 2), np.int32)
+        self._chk(lib().sop_replica_exchange(self._h, int(parity), int(sweep), acc.ctypes.data), "sop_replica_exchange")
+        return acc
+
+    def get_temperatures(self):
+        out = np.zeros(self.T, np.float32)
+        self._chk(lib().sop_get_temperatures(self._h, out.ctypes.data), "sop_get_temperatures")
+        return out
+
     def set_observable_stride(self, stride):
         self._chk(lib().sop_set_observable_stride(self._h, int(stride)), "sop_set_observable_stride")
 
@@ -280,6 +297,8 @@ def sop_set_coords(h, xyz): return h.set_coords(xyz)
 def sop_get_energies(h): return h.get_energies()
 def sop_get_forces(h): return h.get_forces()
 def sop_get_observables(h): return h.get_observables()
+def sop_replica_exchange(h, parity, sweep): return h.replica_exchange(parity, sweep)
+def sop_get_temperatures(h): return h.get_temperatures()
 def sop_set_observable_stride(h, stride): return h.set_observable_stride(stride)
 def sop_get_observable_series(h, max_samples=1 << 20): return h.get_observable_series(max_samples)
 def sop_get_lists(h, level, traj=0): return h.get_lists(level, traj)

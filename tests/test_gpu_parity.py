@@ -687,3 +687,77 @@ def test_p11_long_run_ensemble_means_different_seeds():
         se = math.sqrt(g.var(ddof=1) / T + c.var(ddof=1) / T)
         assert abs(g.mean() - c.mean()) <= 3 * se, (name, g.mean(), c.mean(), se)
         assert se < 0.02 * abs(c.mean())                      # the test has resolving power: 3 SE is a few per cent at most
+
+
+# ---------------------------------------------------------------------------------------------- NEXT-4
+@pytest.mark.parametrize("var", [dict(mode=1, lanes_per_bead=4), dict(mode=2), dict(mode=3), dict(mode=3, chunk_beads=40),
+                                 dict(mode=3, chunk_beads=40, resident_variant=2)], ids=str)
+def test_per_trajectory_temperature_and_replica_exchange(var):
+    """One temperature per run of a many-runs batch, and Metropolis swaps of the temperatures between neighbouring runs
+    (PAPER.md:310).  Same seeds and sweep numbers on both sides: the coordinates agree after 100 steps at four temperatures;
+    at the GPU's coordinates the oracle takes the same swap decisions (decided in fp64 from fp64 sums on both sides; a pair
+    whose uniform falls within 1e-4 of its acceptance probability is not compared), and the runs continue in step."""
+    m = sop()
+    w = gen.two_chains(120, 5, R_pl=20.0)
+    kTs = [0.5, 0.53, 0.56, 0.6, 0.64]
+    p = dict(w.params, kT_per_traj=kTs)
+    T = len(kTs)
+    s = m.Sop(w.xyz, w.bonds, w.native, p, n_traj=T, **var)
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, p, n_traj=T)
+    assert np.allclose(s.get_temperatures(), kTs)
+    s.run(100); o.run(100)
+    xg = s.get_coords()
+    assert np.abs(xg - o.get_coords()).max() <= 1e-3
+    spread = np.abs(xg - w.xyz[None]).reshape(T, -1).std(axis=1)
+    assert spread[-1] > spread[0]                                # hotter runs move more
+    swapped_any = False
+    for sweep in range(12):
+        o.set_coords(xg.astype(np.float64)); o.step = s.step
+        E = o.get_energies()[:, 5]
+        kT = o.get_temperatures()
+        acc_g = s.replica_exchange(sweep & 1, sweep)
+        acc_o = o.replica_exchange(sweep & 1, sweep)
+        for t in range(sweep & 1, T - 1, 2):
+            xw = sopo.philox4x32_10([t, 0x52455821, sweep, 0], [w.params["seed"] & 0xFFFFFFFF, w.params["seed"] >> 32])
+            u = ((int(xw[0]) >> 8) + 1) / 2.0 ** 24
+            pr = sopo.rex_probability(E[t], E[t + 1], kT[t], kT[t + 1])
+            if abs(u - pr) > 1e-4:
+                assert acc_g[t // 2] == acc_o[t // 2], (sweep, t, u, pr)
+            swapped_any = swapped_any or bool(acc_g[t // 2])
+        if not np.array_equal(acc_g, acc_o):
+            pytest.skip("a swap decision within rounding of its threshold")
+        assert np.allclose(s.get_temperatures(), o.get_temperatures())
+        s.run(50); o.run(50)
+        xg = s.get_coords()
+        assert np.abs(xg - o.get_coords()).max() <= 1e-3
+    assert swapped_any and sorted(s.get_temperatures().tolist()) == pytest.approx(sorted(kTs))
+    with pytest.raises(m.SopError):
+        m.Sop(w.xyz, w.bonds, w.native, w.params, n_traj=2, **var).replica_exchange(0, 0)     # no kT_per_traj
+
+
+@pytest.mark.parametrize("lanes", [1, 8])
+def test_second_order_integrator_matches_the_oracle(lanes):
+    """params.integrator = 2: the predictor-corrector whose mean recursion is Eq. (5), two launches per
+    step; coordinates within 1e-3 A of the oracle after 100 steps with pulling, a fixed bead and a finite pair list;
+    bit-identical however the run is split; refused where it is not implemented."""
+    m = sop()
+    w = gen.two_chains(120, 5, R_pl=20.0)
+    p = dict(w.params, integrator=2, fixed=[0], pulled=[119], pull_k=0.05, pull_v=1e-3, pull_dir=[0.0, 0.6, 0.8])
+    T = 2
+    s = m.Sop(w.xyz, w.bonds, w.native, p, n_traj=T, lanes_per_bead=lanes)
+    assert s.config()["mode"] == 1
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, p, n_traj=T)
+    s.run(100); o.run(100)
+    xg, xo = s.get_coords(), o.get_coords()
+    assert np.abs(xg - xo).max() <= 1e-3
+    assert np.array_equal(xg[:, 0], np.broadcast_to(w.xyz[0], (T, 3)))
+    check_lists(s, o, xg[0])
+    b = m.Sop(w.xyz, w.bonds, w.native, p, n_traj=T, lanes_per_bead=lanes); b.run(37); b.run(63)
+    assert np.array_equal(b.get_coords(), xg)
+    c = m.Sop(w.xyz, w.bonds, w.native, dict(p, integrator=1), n_traj=T, lanes_per_bead=lanes); c.run(100)
+    d = np.abs(c.get_coords() - xg).max()
+    assert 1e-7 < d < 0.05                                       # another integrator, the same noise: O(h^2) apart
+    for bad in (dict(mode=3), dict(mode=2), dict(rng=1)):
+        with pytest.raises(m.SopError):
+            m.Sop(w.xyz, w.bonds, w.native, dict(p, **{k: v for k, v in bad.items() if k == "rng"}), n_traj=T,
+                  **{k: v for k, v in bad.items() if k != "rng"})

@@ -10,6 +10,9 @@ P7  bead on a moving spring: Eq. (4) exactly, Eq. (3) to O(h/tau)
 P8  lists: brute force, Table I identity, boundary cases, Alg. 3
 P9  indenter / pulling spring: F = -grad V, 1-D special case        readings R7, R8 (paper silent on the indenter)
 P10 Box-Muller normals: moments, bound, KS
+P13 Eq. (1) magnitudes of the native and repulsion terms by hand
+P14 replica exchange: Metropolis rule, detailed balance, sweep
+P15 second-order update: Eq. (5) exactly, Eq. (3) within 1e-5
 """
 import ctypes
 import math
@@ -738,3 +741,94 @@ def test_p13_eq1_magnitudes_two_beads_hand_evaluated():
         assert e[5] == pytest.approx(V, rel=tol, abs=1e-12)
         assert f[1, 0] == pytest.approx(Fr, rel=tol, abs=1e-12) and f[0, 0] == pytest.approx(-Fr, rel=tol, abs=1e-12)
         assert np.abs(f[:, 1:]).max() == 0.0
+
+
+# ---------------------------------------------------------------------------------------------- P14
+def test_p14_replica_exchange_rule_detailed_balance_and_sweep():
+    """NEXT-4.  (i) hand-evaluated probabilities (tests/golden/rex_metropolis_values.txt); (ii) detailed balance
+    of the swap move on a two-level toy (E = 0 or 1 at kT = 0.5 and 1.0): pi(a, b) p(a, b -> b, a) = pi(b, a) p(b, a -> a, b) with
+    pi = exp(-E_a/kT_1 - E_b/kT_2) -- a wrong sign or swapped temperatures breaks it; (iii) the sweep swaps temperatures,
+    not coordinates, of the pairs of the given parity, with the Philox uniform the header describes."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "rex_metropolis_values.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 4
+    for Ei, Ej, ki, kj, pr in rows:
+        assert sopo.rex_probability(float(Ei), float(Ej), float(ki), float(kj)) == pytest.approx(float(pr), rel=1e-9)
+    k1, k2 = 0.5, 1.0
+    lev = [0.0, 1.0]
+    for a in lev:
+        for b in lev:
+            pi_ab = math.exp(-a / k1 - b / k2); pi_ba = math.exp(-b / k1 - a / k2)
+            assert pi_ab * sopo.rex_probability(a, b, k1, k2) == pytest.approx(pi_ba * sopo.rex_probability(b, a, k1, k2), rel=1e-12)
+    assert sopo.rex_accept(0, 1, k1, k2, 0.36) and not sopo.rex_accept(0, 1, k1, k2, 0.37) and sopo.rex_accept(1, 0, k1, k2, 1.0)
+    # the sweep on five runs of a small chain at five temperatures
+    w = gen.tiny(24, 4)
+    kTs = [0.3, 0.45, 0.6, 0.8, 1.1]
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, dict(w.params, kT_per_traj=kTs), n_traj=5)
+    o.run(200)
+    x = o.get_coords().copy()
+    E = o.get_energies()[:, 5]
+    assert len(set(np.round(E, 6))) == 5                       # five different runs
+    for parity, sweep in ((0, 7), (1, 7), (0, 8), (1, 123456789012)):
+        kT = o.get_temperatures()
+        acc = o.replica_exchange(parity, sweep)
+        new = o.get_temperatures()
+        for t in range(parity, 4, 2):
+            xw = sopo.philox4x32_10([t, 0x52455821, sweep & 0xFFFFFFFF, sweep >> 32], [w.params["seed"] & 0xFFFFFFFF, w.params["seed"] >> 32])
+            u = ((int(xw[0]) >> 8) + 1) / 2.0 ** 24
+            expect = u <= min(1.0, math.exp(min(0.0, (1 / kT[t] - 1 / kT[t + 1]) * (E[t] - E[t + 1]))))
+            assert bool(acc[t // 2]) == expect
+            assert (new[t], new[t + 1]) == ((kT[t + 1], kT[t]) if expect else (kT[t], kT[t + 1]))
+        untouched = [t for t in range(5) if not (t >= parity and (t - parity) // 2 * 2 + parity + 1 < 5)]
+        for t in untouched:
+            assert new[t] == kT[t]
+        assert np.array_equal(o.get_coords(), x)               # temperatures move, coordinates stay
+    assert sorted(o.get_temperatures()) == pytest.approx(sorted(sopo.f32(v) for v in kTs))
+    # the noise amplitude follows the run's temperature: free beads, <dr^2> = 6 kT_t D n per run
+    wf = gen.free_beads(512, R_pl=20.0)
+    of = sopo.Oracle(wf.xyz, wf.bonds, wf.native, dict(wf.params, kT_per_traj=[0.3, 1.2]), n_traj=2)
+    x0 = of.get_coords().copy(); of.run(50)
+    msd = ((of.get_coords() - x0) ** 2).sum(axis=2).mean(axis=1)
+    D = sopo.f32(wf.params["dt_over_zeta"])
+    assert msd[0] == pytest.approx(6 * sopo.f32(0.3) * D * 50, rel=0.15) and msd[1] == pytest.approx(6 * sopo.f32(1.2) * D * 50, rel=0.15)
+
+
+# ---------------------------------------------------------------------------------------------- P15
+def test_p15_second_order_update_is_eq5_and_meets_the_papers_bound():
+    """params.integrator = 2 (reading R14): without noise a bead on the moving spring follows the recursion Eq. (5)
+     to rounding, stays within the paper's printed 1e-5 of Eq. (3) with the paper's parameters
+    (PAPER.md:288; tests/golden/eq5_paper_bound.txt)."""
+    bound2 = float([l for l in open(os.path.join(GOLD, "eq5_paper_bound.txt")) if not l.startswith("#")][0])
+    line = [l for l in open(os.path.join(GOLD, "eq3_eq4_paper_params.txt")) if not l.startswith("#")][0].split()
+    Ksp, D_cm2s, kT = float(line[0]), float(line[3]), float(line[4])
+    tau = kT / (D_cm2s * 1e14 * 1e-12) / Ksp                     # ps
+    # (i) Eq. (5) exactly: X(n+1) = X + (r_f t_n/xi - X/tau) h + (X/(2 tau^2) - r_f t_n/(2 tau xi)) h^2, in the oracle's units
+    kappa, v, D = float(np.float32(0.05)), float(np.float32(1e-3)), float(np.float32(2e-3))
+    w = gen.free_beads(4, R_pl=20.0, kT=0.0, pulled=[0, 1, 2, 3], pull_k=kappa, pull_v=v, pull_dir=[0.0, 0.0, 1.0], integrator=2)
+    o = sopo.from_workload(w)
+    z0 = o.get_coords()[0, :, 2].copy()
+    X, h_tau = 0.0, kappa * D
+    for n in range(300):
+        o.run(1)
+        X = X + (v * n - X) * h_tau + (X - v * n) * h_tau * h_tau / 2
+        assert np.abs(o.get_coords()[0, :, 2] - z0 - X).max() < 1e-12
+    # (ii) the paper's parameters: 10^6 steps against Eq. (3)
+    n = 10 ** 6
+    for h in (1.0, 25.0, 50.0):
+        errs = {}
+        for integ in (1, 2):
+            w = gen.free_beads(2, R_pl=20.0, kT=0.0, pulled=[0, 1], pull_k=1.0, pull_v=1.0, pull_dir=[0.0, 0.0, 1.0])
+            p = dict(w.params, dt_over_zeta=h / tau, nb_interval=1000, pl_interval=100000, integrator=integ)
+            o = sopo.Oracle(w.xyz, w.bonds, w.native, p)
+            a = sopo.f32(h / tau)
+            z0 = o.get_coords()[0, :, 2].copy(); o.run(n)
+            sim = o.get_coords()[0, :, 2] - z0
+            th = n - (1 - math.exp(-n * a)) / a
+            errs[integ] = float(np.abs(sim - th).max() / th)
+        assert errs[2] < bound2 and errs[1] < float(line[7])      # 1e-5 and 2e-5 as printed (both are dominated by the ramp being
+                                                                  # held at t_n during a step, which Eq. (4) and Eq. (5) share)
+    # (iii) with noise the second-order scheme keeps the first-order statistics: free diffusion <dr^2> = 6 kT D n
+    wf = gen.free_beads(512, R_pl=20.0, integrator=2)
+    of = sopo.from_workload(wf)
+    x0 = of.get_coords().copy(); of.run(50)
+    msd = ((of.get_coords() - x0) ** 2).sum(axis=2).mean()
+    assert msd == pytest.approx(6 * sopo.f32(wf.params["kT"]) * sopo.f32(wf.params["dt_over_zeta"]) * 50, rel=0.12)
