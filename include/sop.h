@@ -81,7 +81,11 @@ typedef struct {
   int32_t block_size;                /* 0 auto; threads per block of the step kernel (multiple of 32) */
   int32_t compensated;               /* 0 auto (on if max|coord| > 512 A), 1 on, 2 off: Kahan-compensated
                                         position update (keeps fp32 coordinates accurate at |x| ~ 10^3 A) */
-  int32_t mode;                      /* 0 auto (3 when the chunk state fits shared memory, else 2), 1 one launch per
+  int32_t pair_atomics;              /* mode 4: 0 unique places + gathering (Alg. 4 + 5), 1 atomicAdd into one accumulator per
+                                        bead (the form the paper anticipates for Fermi) */
+  int32_t mode;                      /* 4 = the paper's interacting-pair based scheme (Alg. 4 + 5): one thread
+                                        per pair, every pair force computed once, two launches per step.
+                                        0 auto (3 when the chunk state fits shared memory, else 2), 1 one launch per
                                         step, 2 persistent streaming kernel (grid barrier per step), 3 SM-resident
                                         persistent kernel: a chunk of beads + halo + its L2 rows live in shared
                                         memory, chunks exchange coordinates through stamped words in L2 */

@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsop.so")
 SOURCES = ["sop.cu"]
-DEPS = ["sop.cu", "sop_device.cuh", "sop_kernels.cuh", "sop_persistent.cuh", "sop_resident.cuh", "sop_resident2.cuh", os.path.join("..", "..", "include", "sop.h")]
+DEPS = ["sop.cu", "sop_device.cuh", "sop_kernels.cuh", "sop_persistent.cuh", "sop_resident.cuh", "sop_resident2.cuh", "sop_pairs.cuh", os.path.join("..", "..", "include", "sop.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC"]
 

@@ -15,6 +15,7 @@
 #include "sop_persistent.cuh"
 #include "sop_resident.cuh"
 #include "sop_resident2.cuh"
+#include "sop_pairs.cuh"
 
 using namespace sop;
 
@@ -34,7 +35,8 @@ struct Plan {                     // everything that depends only on (topology, 
   // workspace offsets
   size_t off_pos0, off_pos1, off_carry, off_force, off_bond, off_natptr, off_nattab, off_nateps, off_exclptr,
       off_exclidx, off_adotn, off_plcnt, off_plidx, off_nbcnt, off_nbidx, off_bbox, off_grid, off_cellof,
-      off_cellcnt, off_cellstart, off_cellbead, off_cellpos, off_taus, off_flags, off_epart, off_eout, off_bar, off_series, off_kTt, off_ampt, off_rexacc, total;
+      off_cellcnt, off_cellstart, off_cellbead, off_cellpos, off_taus, off_flags, off_epart, off_eout, off_bar, off_series, off_kTt, off_ampt, off_rexacc, off_spair, off_spar, off_lpair, off_nlpair, off_F, off_Facc, total;
+  int cap_pairs = 0, n_place = 0;
   // mode 3 (SM-resident kernel): chunking, launch shape, shared-memory carve-up, workspace
   bool res_ok = false;
   std::string res_why;
@@ -78,6 +80,7 @@ struct sop_handle {
  ResDev R;                       // mode 3
   Res2Dev R2;
   const void *res2_fn = nullptr;
+  PairDev P;                      // mode 4
   int64_t obs_stride = 0, obs_count = 0;   // observables recorded every obs_stride steps into a device ring of obs_cap samples
   int obs_cap = 0;
   std::vector<int64_t> obs_steps;           // [obs_cap] step of the sample in every ring slot
@@ -454,9 +457,10 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.lanes = lanes;
   pl.block = p->block_size > 0 ? p->block_size : 256;
   if (pl.block % 32 || pl.block > 1024) return fail(SOP_E_ARG, "block_size must be a multiple of 32, <= 1024");
-  if (p->mode < 0 || p->mode > 3) return fail(SOP_E_ARG, "mode must be 0, 1, 2 or 3");
+  if (p->mode < 0 || p->mode > 4) return fail(SOP_E_ARG, "mode must be 0 ... 4");
+  if (p->mode == 4 && p->rng != 0) return fail(SOP_E_ARG, "mode 4 (pair based) runs with rng = 0");
   if (p->integrator < 0 || p->integrator > 2) return fail(SOP_E_ARG, "integrator must be 0, 1 or 2");
-  if (p->integrator == 2 && (p->rng != 0 || p->mode > 1))
+  if (p->integrator == 2 && (p->rng != 0 || (p->mode > 1)))
     return fail(SOP_E_ARG, "integrator = 2 (second order, Eq. (5)) runs in mode 1 with rng = 0");
   if (p->kT_per_traj)
     for (int t = 0; t < T; ++t)
@@ -506,6 +510,15 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
   pl.off_kTt = take(p->kT_per_traj ? (size_t)T * 4 : 0);
   pl.off_ampt = take(p->kT_per_traj ? (size_t)T * 4 : 0);
   pl.off_rexacc = take(p->kT_per_traj ? (size_t)T * 4 : 0);
+  if (pl.mode == 4) {                 // the pair-based scheme (sop_pairs.cuh): pair vectors and the array of force places
+    const size_t n_static = (size_t)tp->n_bonds + (size_t)tp->n_native;
+    pl.cap_pairs = (int)std::min<size_t>(0x7FFFFFF0, ((size_t)N * pl.cap_nb + 1) / 2);
+    pl.n_place = (int)((size_t)N * pl.cap_b + pl.n_nat_entries + (size_t)N * pl.cap_nb);
+    pl.off_spair = take(n_static * 16); pl.off_spar = take(n_static * 8);
+    pl.off_lpair = take((size_t)T * pl.cap_pairs * 16); pl.off_nlpair = take((size_t)T * 4);
+    pl.off_F = take(p->pair_atomics ? 0 : (size_t)T * pl.n_place * 16);
+    pl.off_Facc = take(p->pair_atomics ? I * 16 : 0);
+  }
   if (pl.mode == 3) {
     const ResDev &R = pl.R;
     const bool multi = R.C > 1;
@@ -567,6 +580,20 @@ void launch_step(sop_handle *h, bool forces) {
   }
 }
 
+// mode 4: Alg. 4 (thread per pair) + Alg. 5 fused with the update (thread per bead)
+void launch_pair_step(sop_handle *h, bool forces) {
+  const SysDev &S = h->S;
+  const PairDev &P = h->P;
+  const unsigned gp = (unsigned)(((long long)P.n_static + P.cap_pairs + 255) / 256);
+  k_pair_forces<<<dim3(gp, (unsigned)S.T), 256, 0, h->stream>>>(S, P, h->cur);
+  const unsigned gb = (unsigned)((S.n_inst + 255) / 256);
+  const unsigned long long step = (unsigned long long)h->step;
+  if (forces) k_pair_gather_update<false, true><<<gb, 256, 0, h->stream>>>(S, P, h->cur, step);
+  else if (h->plan.comp) k_pair_gather_update<true, false><<<gb, 256, 0, h->stream>>>(S, P, h->cur, step);
+  else k_pair_gather_update<false, false><<<gb, 256, 0, h->stream>>>(S, P, h->cur, step);
+  h->launches += 2;
+}
+
 template <int G>
 void launch_step2_g(sop_handle *h, int stage) {
   const SysDev &S = h->S;
@@ -595,6 +622,11 @@ void launch_filter(sop_handle *h) {
   const long long threads = (long long)S.n_inst * 32;
   k_filter<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(S, h->cur);
   h->launches++;
+  if (h->plan.mode == 4) {            // the vector of L2 pairs follows the neighbor list
+    cudaMemsetAsync(h->P.n_lpair, 0, (size_t)S.T * 4, h->stream);
+    k_pairs_build<<<(unsigned)((threads + 255) / 256), 256, 0, h->stream>>>(S, h->P);
+    h->launches++;
+  }
   h->l2_built_at = h->step;
 }
 
@@ -905,6 +937,25 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
     excl_ptr[i + 1] = (int)excl_idx.size();
   }
 
+  // ---- mode 4: the static pairs of Alg. 4 (every bond and native contact once) with their places in the force array
+  std::vector<int4> spair;
+  std::vector<float2> spar;
+  if (pl.mode == 4) {
+    auto bond_slot = [&](int ii, int jj) { for (int b = 0; b < pl.cap_b; ++b) if (bond_tab[(size_t)ii * pl.cap_b + b].x == jj) return ii * pl.cap_b + b; return -1; };
+    auto nat_slot = [&](int ii, int jj) { for (int q = nat_ptr[ii]; q < nat_ptr[ii + 1]; ++q) if (nat_tab[q].x == jj) return N * pl.cap_b + q; return -1; };
+    for (int b = 0; b < tp->n_bonds; ++b) {
+      const int ii = pl.iperm[tp->bonds[2 * b]], jj = pl.iperm[tp->bonds[2 * b + 1]];
+      spair.push_back(make_int4(ii, jj, bond_slot(ii, jj), bond_slot(jj, ii)));
+      spar.push_back(make_float2((float)dist(tp->bonds[2 * b], tp->bonds[2 * b + 1]), 0.f));
+    }
+    for (int c = 0; c < tp->n_native; ++c) {
+      const int ii = pl.iperm[tp->native[2 * c]], jj = pl.iperm[tp->native[2 * c + 1]];
+      const float r0 = (float)dist(tp->native[2 * c], tp->native[2 * c + 1]);
+      spair.push_back(make_int4(ii, jj, nat_slot(ii, jj), nat_slot(jj, ii)));
+      spar.push_back(make_float2((float)((double)r0 * (double)r0), tp->native_eps ? tp->native_eps[c] : p->eps_native));
+    }
+  }
+
   // ---- tags, anchors, initial coordinates
   std::vector<uint32_t> &tag = h->tag;
   tag.resize(N);
@@ -997,6 +1048,17 @@ int sop_create(const sop_topology *tp, const float *native_xyz, const sop_params
     for (int t = 0; t < T; ++t) { kT_t.push_back(p->kT_per_traj[t]); amp_t.push_back((float)std::sqrt(2.0 * (double)p->kT_per_traj[t] * (double)p->dt_over_zeta)); }
     acc(up(pl.off_kTt, kT_t.data(), (size_t)T * 4)); acc(up(pl.off_ampt, amp_t.data(), (size_t)T * 4));
   }
+  if (pl.mode == 4) {
+    PairDev &P = h->P;
+    memset(&P, 0, sizeof(P));
+    P.n_static = (int)spair.size(); P.n_bonds = tp->n_bonds;
+    P.spair = (const int4 *)(w + pl.off_spair); P.spar = (const float2 *)(w + pl.off_spar);
+    P.cap_pairs = pl.cap_pairs; P.lpair = (int4 *)(w + pl.off_lpair); P.n_lpair = (int *)(w + pl.off_nlpair);
+    P.n_place = pl.n_place; P.F = (float4 *)(w + pl.off_F); P.Facc = (float *)(w + pl.off_Facc); P.atomics = p->pair_atomics ? 1 : 0;
+    acc(up(pl.off_spair, spair.data(), spair.size() * 16)); acc(up(pl.off_spar, spar.data(), spar.size() * 8));
+    acc(cudaMemsetAsync(w + pl.off_nlpair, 0, (size_t)T * 4, st));
+    if (P.atomics) acc(cudaMemsetAsync(w + pl.off_Facc, 0, (size_t)N * T * 16, st));
+  }
   acc(cudaStreamSynchronize(st));
   if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); delete h; return fail(SOP_E_CUDA, "upload: " + m); }
 
@@ -1069,7 +1131,7 @@ int sop_run(sop_handle *h, int64_t n_steps) {
   int64_t left = n_steps;
   bool pending_filter = false;
   while (left > 0) {
-    if (h->plan.mode >= 2) {
+    if (h->plan.mode == 2 || h->plan.mode == 3) {
       // one persistent launch runs up to the next pair-list boundary (or observable sample), re-filtering L2 inside
       int64_t n = std::min<int64_t>(left, (1 << 20) - 2);
       if (!h->S.static_l1) n = std::min<int64_t>(n, plv - (h->step % plv));
@@ -1093,7 +1155,7 @@ int sop_run(sop_handle *h, int64_t n_steps) {
     } else {
       span_begin(h, SPAN_STEP, 1);
       if (h->prm.integrator == 2) { launch_step2(h, 0); launch_step2(h, 1); h->step++; left--; }     // (the result is back in layer cur)
-      else { launch_step(h, false); h->cur ^= 1; h->step++; left--; }
+      else { if (h->plan.mode == 4) launch_pair_step(h, false); else launch_step(h, false); h->cur ^= 1; h->step++; left--; }
       if (!h->S.static_l1 && h->step % plv == 0) { int rc = launch_build_l1(h); if (rc) return rc; }
       if (h->step % nb == 0) launch_filter(h);
       if (ost > 0 && h->step % ost == 0) { int rc = record_sample(h); if (rc) return rc; }
@@ -1262,7 +1324,7 @@ int sop_get_forces(sop_handle *h, float *f_out) {
   const int N = h->S.N, T = h->S.T;
   int rc = ensure_stage(h);
   if (rc) return rc;
-  launch_step(h, true);
+  if (h->plan.mode == 4) launch_pair_step(h, true); else launch_step(h, true);
   rc = check_launch(h, "forces");
   if (rc) return rc;
   CUDA_OK(cudaMemcpyAsync(h->stage, h->S.force, (size_t)N * T * 16, cudaMemcpyDeviceToHost, h->stream));

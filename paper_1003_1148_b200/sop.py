@@ -43,7 +43,7 @@ class _Params(C.Structure):
                 ("tip_on", C.c_int32), ("tip_R", C.c_float), ("tip_eps", C.c_float), ("tip_sigma", C.c_float),
                 ("tip_c0", C.c_float * 3), ("tip_dir", C.c_float * 3), ("tip_v", C.c_float),
                 ("lanes_per_bead", C.c_int32), ("block_size", C.c_int32), ("compensated", C.c_int32),
-                ("mode", C.c_int32), ("reorder", C.c_int32), ("chunk_beads", C.c_int32), ("resident_variant", C.c_int32),
+                ("pair_atomics", C.c_int32), ("mode", C.c_int32), ("reorder", C.c_int32), ("chunk_beads", C.c_int32), ("resident_variant", C.c_int32),
                 ("obs_stride", C.c_int32), ("obs_capacity", C.c_int32), ("rng", C.c_int32),
                 ("stream", C.c_void_p)]
 
@@ -133,6 +133,7 @@ def _marshal(xyz, bonds, native, params, native_eps, overrides):
     pp.tip_dir = (C.c_float * 3)(*[float(v) for v in p.get("tip_dir", [0, 0, -1])])
     pp.tip_v = float(p.get("tip_v", 0.0))
     pp.lanes_per_bead = int(p.get("lanes_per_bead", 0)); pp.block_size = int(p.get("block_size", 0))
+    pp.pair_atomics = int(p.get("pair_atomics", 0))
     pp.compensated = int(p.get("compensated", 0)); pp.mode = int(p.get("mode", 0)); pp.reorder = int(p.get("reorder", 0))
     pp.chunk_beads = int(p.get("chunk_beads", 0)); pp.rng = int(p.get("rng", 0))
     pp.resident_variant = int(p.get("resident_variant", 0))

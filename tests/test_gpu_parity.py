@@ -76,7 +76,8 @@ VARIANTS = [dict(mode=1, lanes_per_bead=1), dict(mode=1, lanes_per_bead=8), dict
             dict(mode=2, lanes_per_bead=4), dict(mode=2, lanes_per_bead=16, reorder=1), dict(mode=1, reorder=1),
             dict(mode=3), dict(mode=3, chunk_beads=40, lanes_per_bead=4), dict(mode=3, chunk_beads=64, lanes_per_bead=1),
             dict(mode=3, chunk_beads=33, lanes_per_bead=16, compensated=1),
-            dict(mode=3, chunk_beads=40, resident_variant=2), dict(mode=3, chunk_beads=64, resident_variant=2, compensated=1)]
+            dict(mode=3, chunk_beads=40, resident_variant=2), dict(mode=3, chunk_beads=64, resident_variant=2, compensated=1),
+            dict(mode=4), dict(mode=4, pair_atomics=1), dict(mode=4, reorder=1, compensated=1)]
 
 
 @pytest.mark.parametrize("name,make,over", SMALL, ids=[c[0] for c in SMALL])
@@ -761,3 +762,42 @@ def test_second_order_integrator_matches_the_oracle(lanes):
         with pytest.raises(m.SopError):
             m.Sop(w.xyz, w.bonds, w.native, dict(p, **{k: v for k, v in bad.items() if k == "rng"}), n_traj=T,
                   **{k: v for k, v in bad.items() if k != "rng"})
+
+
+# ---------------------------------------------------------------------------------------------- NEXT-3: pair-based scheme
+@pytest.mark.parametrize("atomics", [0, 1])
+def test_pair_based_scheme_mode4(atomics):
+    """Alg. 4 + Alg. 5: one thread per pair, forces saved to unique places and gathered in the update
+    kernel (atomics = 0), or added atomically (atomics = 1, the form the paper anticipates).  Forces, lists,
+    energies and 100-step coordinates against the oracle with pulling, an indenter, per-contact eps and a batch; the
+    unique-place form is bit-identical run to run and however the run is split."""
+    m = sop()
+    w = gen.two_chains(150, 3, R_pl=20.0)
+    zmax = float(w.xyz[:, 2].max())
+    eps = (0.5 + np.random.default_rng(9).random(len(w.native))).astype(np.float32)
+    p = dict(w.params, fixed=[0, 5], pulled=[149], pull_k=0.05, pull_v=1e-3, pull_dir=[0.6, 0.0, 0.8],
+             tip_on=1, tip_R=50.0, tip_eps=1.0, tip_sigma=3.8, tip_c0=[0.0, 0.0, zmax + 53.0], tip_dir=[0.0, 0.0, -1.0], tip_v=1e-3)
+    T = 3
+    s = m.Sop(w.xyz, w.bonds, w.native, p, n_traj=T, native_eps=eps, mode=4, pair_atomics=atomics)
+    o = sopo.Oracle(w.xyz, w.bonds, w.native, p, n_traj=T, native_eps=eps)
+    assert s.config()["mode"] == 4
+    f_gpu, f_cpu = s.get_forces(), o.get_forces()
+    assert np.abs(f_gpu - f_cpu).max() <= 1e-4 * np.abs(f_cpu).max()
+    check_energies(s.get_energies(), o.get_energies())
+    s.run(100); o.run(100)
+    xg = s.get_coords()
+    assert np.abs(xg - o.get_coords()).max() <= 1e-3
+    check_lists(s, o, xg[T - 1], traj=T - 1)
+    b = m.Sop(w.xyz, w.bonds, w.native, p, n_traj=T, native_eps=eps, mode=4, pair_atomics=atomics); b.run(37); b.run(63)
+    if atomics == 0:
+        assert np.array_equal(b.get_coords(), xg)                  # unique places: no dependence on the order of the pairs
+    else:
+        assert np.abs(b.get_coords() - xg).max() < 1e-4            # atomic additions: the order of the sum is not fixed
+    # against the particle-based kernels: the same pair terms, summed in another order
+    c = m.Sop(w.xyz, w.bonds, w.native, p, n_traj=T, native_eps=eps, mode=1, lanes_per_bead=1); c.run(100)
+    assert np.abs(c.get_coords() - xg).max() < 1e-4
+
+
+def test_pair_based_scheme_full_config0_and_3():
+    full_check(0, mode=4)
+    full_check(3, mode=4)
