@@ -154,6 +154,37 @@ def algorithmic_bytes(st, T, compensated, static_l1, p):
     return {"B_fi": b_fi, "B_filter": b_filter, "B_l1": b_l1, "B_step": per_step}
 
 
+def roofline_block(res, w, T, peak, peak_src):
+    """The roofline record of one measured workload: algorithmic bytes / CUDA-event time of the step kernel /
+    measured HBM copy peak, with every term it is made of, and the DRAM traffic of the committed ncu capture beside it."""
+    sk = res.get("step_kernel")
+    if not sk:
+        return None
+    ab, nbi = res["bytes"], w.params["nb_interval"]
+    inside = sk["includes_l2_filter"]
+    per_bead_step = ab["B_fi"] + (ab["B_filter"] / nbi if inside else 0.0)
+    out = {"bound": "hbm",
+           "kernel": "fused force+noise+update step kernel" + (" (persistent; L2 filter inside)" if inside else ""),
+           "achieved": sk["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": sk["achieved_gbs"] / peak, "peak_source": peak_src,
+           "frac_is": "ALGORITHMIC bytes / time / measured HBM copy peak (the working set is SM/L2 resident: see dram_frac and limited_by)",
+           "frac_of_nominal_8TBs": sk["achieved_gbs"] / NOMINAL_HBM_GBS, "us_per_langevin_step": sk["us_per_langevin_step"],
+           "bytes_per_bead_step": per_bead_step, "B_fi": ab["B_fi"], "B_filter_per_step": ab["B_filter"] / nbi if inside else 0.0,
+           "bead_instances": w.n_beads * T, "traffic": None, "traffic_source": None, "algorithmic_bytes_per_launch": None}
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.json.txt")) as f:
+            tr = json.load(f).get(w.name)
+        if tr and res["resolved"]["mode"] == tr["mode"]:
+            out["traffic"] = tr["dram_bytes_per_launch"]
+            out["traffic_source"] = (f"ncu dram__bytes_read.sum + dram__bytes_write.sum of one {tr['kernel']} launch = "
+                                     f"{tr['langevin_steps_per_launch']} Langevin steps ({tr['profile']})")
+            out["algorithmic_bytes_per_launch"] = per_bead_step * w.n_beads * T * tr["langevin_steps_per_launch"]
+            out["dram_frac"] = tr["dram_bytes_per_launch"] / (tr["langevin_steps_per_launch"] * sk["us_per_langevin_step"] * 1e-6) / 1e9 / peak
+            out["limited_by"] = tr.get("limited_by")
+    except Exception:  # noqa: BLE001
+        pass
+    return out
+
+
 # ---------------------------------------------------------------------------------------------- our arm
 def measure(w, T, traj_offset, block, K, W, clocks_index=None, e2e=True, overrides=None):
     """Time K bench steps of `block` Langevin steps (+ one energy reduction) on the current device."""
@@ -197,14 +228,14 @@ def measure(w, T, traj_offset, block, K, W, clocks_index=None, e2e=True, overrid
     ab = algorithmic_bytes(st, T, cfg["compensated"], math.isinf(w.params["R_pl"]), w.params)
     res = {
         "value": units / (ms_max * 1e-3), "ms_per_step": ms_max / K, "us_per_langevin_step": ms_max * 1e3 / (K * block),
-        "launches": int(launches), "resolved": {k: cfg[k] for k in ("lanes_per_bead", "block_size", "compensated", "mode", "reorder")},
+        "launches": int(launches), "resolved": {k: cfg[k] for k in ("lanes_per_bead", "block_size", "compensated", "mode", "reorder", "resident_variant")},
         "list_stats": st, "bytes": ab, "profile": prof,
     }
     # force+integrate kernel alone (its own event spans inside the library, on the same stream)
     if prof["langevin_steps"] > 0 and prof["step_ms"] > 0:
         us_fi = prof["step_ms"] * 1e3 / prof["langevin_steps"]
-        n_filters_inside = prof["langevin_steps"] // w.params["nb_interval"] if cfg["mode"] >= 2 else 0
-        bytes_per_launch_step = N * T * (ab["B_fi"] + (ab["B_filter"] / w.params["nb_interval"] if cfg["mode"] >= 2 else 0.0))
+        n_filters_inside = prof["langevin_steps"] // w.params["nb_interval"] if cfg["mode"] in (2, 3) else 0
+        bytes_per_launch_step = N * T * (ab["B_fi"] + (ab["B_filter"] / w.params["nb_interval"] if cfg["mode"] in (2, 3) else 0.0))
         res["step_kernel"] = {"us_per_langevin_step": us_fi, "achieved_gbs": bytes_per_launch_step / (us_fi * 1e-6) / 1e9,
                               "includes_l2_filter": bool(n_filters_inside), "spans": prof["step_spans"]}
     if sampler:
@@ -264,6 +295,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--mode", type=int, default=0)
     ap.add_argument("--lanes", type=int, default=0)
+    ap.add_argument("--variant", type=int, default=0, help="mode 3 with several chunks: resident_variant (1 first design, 2 second design)")
     ap.add_argument("--sweep4", action="store_true",
                     help="config 4's sweep of the parallelisation variant (BASELINE.json configs[4]): lanes per bead x block size")
     args = ap.parse_args()
@@ -310,6 +342,8 @@ def main():
         over["mode"] = args.mode
     if args.lanes:
         over["lanes_per_bead"] = args.lanes
+    if args.variant:
+        over["resident_variant"] = args.variant
     w = gen.make_config(args.config)
     T = w.n_traj
     peak, peak_src = measured_peak()
@@ -326,26 +360,9 @@ def main():
                    **main_res["resolved"]},
         "e2e": main_res.get("e2e"), "gpu_launches": main_res["launches"], "clocks": main_res.get("clocks"),
     }
-    sk = main_res.get("step_kernel")
-    # dram traffic of the dominant kernel per launch, from the committed ncu --set full capture (profiles/), or null
-    traffic = traffic_src = alg_per_launch = None
-    try:
-        with open(os.path.join(ROOT, "profiles", "r1p_traffic.json.txt")) as f:
-            tr = json.load(f).get(w.name)
-        if tr and main_res["resolved"]["mode"] == 3:
-            traffic = tr["dram_bytes_per_launch"]
-            traffic_src = f"ncu dram__bytes_read.sum + dram__bytes_write.sum of one {tr['kernel']} launch = {tr['langevin_steps_per_launch']} Langevin steps (profiles/r1p_ncu_cfg3_resident.md)"
-            alg_per_launch = (main_res["bytes"]["B_fi"] + main_res["bytes"]["B_filter"] / w.params["nb_interval"]) * w.n_beads * T * tr["langevin_steps_per_launch"]
-    except Exception:  # noqa: BLE001
-        pass
-    if sk:
-        line["roofline"] = {
-            "bound": "hbm", "kernel": "fused force+noise+update step kernel" + (" (persistent; L2 filter inside)" if sk["includes_l2_filter"] else ""),
-            "achieved": sk["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": sk["achieved_gbs"] / peak, "peak_source": peak_src,
-            "frac_of_nominal_8TBs": sk["achieved_gbs"] / NOMINAL_HBM_GBS, "us_per_langevin_step": sk["us_per_langevin_step"],
-            "bytes_per_bead_step": main_res["bytes"]["B_fi"], "traffic": traffic, "traffic_source": traffic_src,
-            "algorithmic_bytes_per_launch": alg_per_launch,
-            "note": "algorithmic bytes / CUDA-event time of the step kernel; the working set is L2/SM resident, so dram traffic is far below the algorithmic bytes (profiles/)"}
+    rl = roofline_block(main_res, w, T, peak, peak_src)
+    if rl:
+        line["roofline"] = rl
     pr = main_res["profile"]
     line["list_kernels"] = {
         "l1_rebuild_us": pr["l1_ms"] * 1e3 / pr["l1_spans"] if pr["l1_spans"] else None, "l1_rebuilds": pr["l1_spans"],
@@ -354,6 +371,7 @@ def main():
         "note": "CUDA-event spans inside the library: a1+a2 (+ slot localisation in mode 3) per pair-list rebuild; a3 as its own "
                 "kernel (modes 2/3 filter inside the step kernel, so only the end-of-run / set_coords filters show up here)"}
     line["whole_step_gbs"] = main_res["bytes"]["B_step"] * w.n_beads * T * world / (main_res["us_per_langevin_step"] * 1e-6) / 1e9
+    line["whole_step_frac"] = line["whole_step_gbs"] / world / peak
 
     if rank == 0 and world == 1:
         if not args.no_sweep:
@@ -368,8 +386,43 @@ def main():
                                   "step_kernel_us": r.get("step_kernel", {}).get("us_per_langevin_step"),
                                   "step_kernel_gbs": r.get("step_kernel", {}).get("achieved_gbs"),
                                   "step_kernel_frac": r.get("step_kernel", {}).get("achieved_gbs", 0.0) / peak,
+                                  "whole_path_gbs": r["bytes"]["B_step"] * wk.n_beads * wk.n_traj / (r["us_per_langevin_step"] * 1e-6) / 1e9,
+                                  "whole_path_frac": r["bytes"]["B_step"] * wk.n_beads * wk.n_traj / (r["us_per_langevin_step"] * 1e-6) / 1e9 / peak,
+                                  "l1_rebuild_us": r["profile"]["l1_ms"] * 1e3 / r["profile"]["l1_spans"] if r["profile"]["l1_spans"] else None,
+                                  "standalone_filter_us": r["profile"]["filter_ms"] * 1e3 / r["profile"]["filter_spans"] if r["profile"]["filter_spans"] else None,
+                                  "roofline": roofline_block(r, wk, wk.n_traj, peak, peak_src),
                                   "B_fi": r["bytes"]["B_fi"], **r["resolved"]}
             line["workloads"] = sweep
+            # variants of the path on the same inputs: the paper's pair-based scheme (mode 4, NEXT-3) on cfg 0 and cfg 3, the
+            # second resident kernel (resident_variant 2) on cfg 2 and cfg 3, the paper's Hybrid Taus generator (rng 1) on cfg 3
+            var = {}
+            for name, k, ov in (("cfg0_mode4_pair_based", 0, {"mode": 4}), ("cfg0_mode4_pair_based_atomics", 0, {"mode": 4, "pair_atomics": 1}),
+                                ("cfg3_mode4_pair_based", 3, {"mode": 4}), ("cfg3_mode1_particle_based", 3, {"mode": 1}),
+                                ("cfg3_resident_variant2", 3, {"resident_variant": 2}), ("cfg2_resident_variant2", 2, {"resident_variant": 2}),
+                                ("cfg3_hybrid_taus", 3, {"rng": 1})):
+                wk = gen.make_config(k)
+                blk = 1000 if ov.get("mode", 3) == 3 or k == 0 else 200
+                r = measure(wk, wk.n_traj, 0, blk, 2, 3, e2e=False, overrides=ov)
+                var[name] = {"us_per_langevin_step": r["us_per_langevin_step"], "step_kernel_us": r.get("step_kernel", {}).get("us_per_langevin_step"),
+                             "value": r["value"], **r["resolved"]}
+            line["variants"] = var
+            # the host side of the getters at the many-runs size (256,000 bead instances): pinned staging + index permutation
+            import time as _t
+            import paper_1003_1148_b200 as m
+            w1 = gen.make_config(1)
+            s1 = m.from_workload(w1)
+            x1 = s1.get_coords()
+            t0 = _t.perf_counter()
+            for _ in range(5):
+                s1.get_coords(out=x1)
+            t1 = _t.perf_counter()
+            for _ in range(5):
+                s1.set_coords(x1)
+            s1.sync()
+            t2 = _t.perf_counter()
+            line["host_io_cfg1"] = {"get_coords_ms": (t1 - t0) / 5 * 1e3, "set_coords_ms_incl_list_rebuild": (t2 - t1) / 5 * 1e3,
+                                    "bead_instances": w1.n_beads * w1.n_traj}
+            s1.close()
         if args.sweep4:
             # thread-per-bead (1 lane) ... warp-per-bead (32 lanes) x the paper's block sizes, mode 1
             w4 = gen.make_config(4)

@@ -86,7 +86,7 @@ __device__ __forceinline__ bool xch_try(const uint4 *slot, uint32_t st, float4 &
 // to time and gives up too, so the cooperative launch ends with an error status instead of hanging the GPU.
 constexpr int FLAG_EXCHANGE_TIMEOUT = 32;
 constexpr unsigned XCH_SPIN_LIMIT = 1u << 23;
-__device__ __noinline__ bool xch_slow_wait(const uint4 *slot, uint32_t st, float4 &out, int *flags) {
+__device__ __forceinline__ bool xch_slow_wait(const uint4 *slot, uint32_t st, float4 &out, int *flags) {
   volatile int *abort_word = flags + 1;
   for (unsigned spins = 0;; ++spins) {
     if (xch_try(slot, st, out)) return true;

@@ -436,6 +436,13 @@ __global__ void __launch_bounds__(1024, 1) k_res2(SysDev S, ResDev R, Res2Dev Q,
   auto filter_rows = [&](const float4 *ownp, const float4 *halop, bool member) {
     const float R2 = S.R_nb2;
     unsigned long long mo[R2_MAXR], mh[R2_MAXR];
+    // the rows are in the order of their force-row sizes, which follow the L1 row sizes: odd rounds walk their block of rows
+    // backwards, so that a quarter-warp that got a short row in one round gets a long one in the next
+    auto row_of = [&](int r) {
+      const int first = r * nqw, last = min(n_own, first + nqw) - 1;
+      const int ix = (r & 1) ? last - qw : first + qw;
+      return ix >= first && ix <= last ? ix : -1;
+    };
     const int bm_words = (Q.own_stride + Q.halo_stride + 31) >> 5;      // membership bitmap of one row (scratch in the row region)
     uint32_t *mbm = (uint32_t *)rows + (size_t)qw * bm_words;
     auto test_segment = [&](const unsigned short *row, int G, const float4 *P4, int pad, const float4 &ri, int bit0) {
@@ -465,8 +472,9 @@ __global__ void __launch_bounds__(1024, 1) k_res2(SysDev S, ResDev R, Res2Dev Q,
     for (int r = 0; r < R2_MAXR; ++r) {
       mo[r] = 0ull; mh[r] = 0ull;
       if (r * nqw < n_own) {
-        const bool valid = r * nqw + qw < n_own;
-        const int il = order[valid ? r * nqw + qw : n_own - 1];
+        const int ix = row_of(r);
+        const bool valid = ix >= 0;
+        const int il = order[valid ? ix : n_own - 1];
         const size_t g = inst0 + b0 + il;
         const uchar2 gg = valid ? Q.pl_g[g] : make_uchar2(0, 0);
         const unsigned short *row = Q.pl_arr + g * Q.cap_arr + l8;
@@ -502,8 +510,9 @@ __global__ void __launch_bounds__(1024, 1) k_res2(SysDev S, ResDev R, Res2Dev Q,
 #pragma unroll
     for (int r = 0; r < R2_MAXR; ++r) {
       if (r * nqw < n_own && fits) {
-        const bool valid = r * nqw + qw < n_own;
-        const int il = order[valid ? r * nqw + qw : n_own - 1];
+        const int ix = row_of(r);
+        const bool valid = ix >= 0;
+        const int il = order[valid ? ix : n_own - 1];
         const size_t g = inst0 + b0 + il;
         const uchar2 gg = valid ? Q.pl_g[g] : make_uchar2(0, 0);
         const unsigned short *row = Q.pl_arr + g * Q.cap_arr + l8, *rowh = row + 8 * gg.x;
