@@ -42,7 +42,7 @@ struct Plan {                     // everything that depends only on (topology, 
   std::string res_why;
   int res_lanes = 1, res_block = 1024, res_nat_rows = 0;
   ResDev R;
-  size_t off_nhalo, off_hgid, off_plloc, off_natloc, off_bondloc, off_xch, off_xchf;
+  size_t off_nhalo, off_hgid, off_plloc, off_natloc, off_bondloc, off_xch, off_xchf, off_nbglob;
   // mode 3, several chunks per trajectory: the second resident kernel (sop_resident2.cuh) when its plan fits
   bool res2_ok = false;
   int res2_block = 0;
@@ -315,28 +315,29 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
   R.nb_si = pl.cap_nb + 4;                       // rows padded to a multiple of four slots, 8-byte aligned
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = (o + bytes + 15) / 16 * 16; return (int)at; };
-  auto carve = [&](bool nat_smem, int pl_cap) {
+  auto carve = [&](bool nat_smem, int pl_cap, bool stream = false) {
     o = 0;
     R.nat_smem = nat_smem ? 1 : 0;
     R.pl_cap = pl_cap;
-    R.off_pos = take(2 * (size_t)(slots + 1) * 16);
+    R.stream = stream ? 1 : 0;
+    R.off_pos = take((stream ? 1 : 2) * (size_t)(slots + 1) * 16);
     R.off_g = take(G > 1 ? 2 * (size_t)chunk * 16 : 0);
     R.off_carry = take(pl.comp ? (size_t)chunk * 16 : 0);
     R.off_tag = take((size_t)chunk * 4);
     R.off_force = take((size_t)chunk * 16);
-    R.off_nb = take((size_t)chunk * R.nb_si * 2);
+    R.off_nb = take(stream ? 0 : (size_t)chunk * R.nb_si * 2);
     R.off_cnt = take((size_t)chunk * 2);
     R.off_plcnt = take((size_t)chunk * 2);
-    R.off_plofs = take(((size_t)chunk + 1) * 4);
+    R.off_plofs = take(stream ? 0 : ((size_t)chunk + 1) * 4);
     R.off_pl = take((size_t)pl_cap * 2);
     R.off_natq = take(((size_t)chunk + 1) * 4);
     R.off_nat = take(nat_smem ? (size_t)R.nat_cap * 8 : 0);
-    R.off_bond = take((size_t)chunk * pl.cap_b * 8);
-    R.off_active = take((size_t)halo_cap * 2);
+    R.off_bond = take(stream ? 0 : (size_t)chunk * pl.cap_b * 8);
+    R.off_active = take(stream ? 0 : (size_t)halo_cap * 2);
     R.off_bm = take((size_t)(halo_cap / 32 + 1) * 4);
     R.off_sbm = take((size_t)(halo_cap / 32 + 1) * 4);
     R.off_misc = take(64);
-    R.off_order = take((size_t)chunk * 2);
+    R.off_order = take(stream ? 0 : (size_t)chunk * 2);
     R.off_hist = take(64 * 4);
     R.smem_bytes = (int)o;
   };
@@ -354,7 +355,13 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
     if (left > 4 * chunk) carve(nat_ok, (int)std::min<long long>(pl_want, left));
   }
   if (o > 232448 && !pl.static_l1) carve(false, 0);
-  if (o > 232448) { pl.res_why = "chunk state does not fit the 227 KB of shared memory of an SM"; return; }
+  // still too large (chunks of a thousand beads and more): keep only the coordinates resident and stream the lists
+  if (o > 232448 && !pl.static_l1 && C > 1 && G <= 2) carve(false, 0, true);
+  if (getenv("SOP_TEST_STREAM") && !pl.static_l1 && C > 1 && G <= 2) carve(false, 0, true);   // test hook: the streamed variant on small inputs
+  if (o > 232448) {
+    if (getenv("SOP_DEBUG_PLAN")) fprintf(stderr, "[sop plan] mode 3 does not fit: C=%d chunk=%d lanes=%d halo_cap=%d smem=%zu B\n", C, chunk, G, halo_cap, o);
+    pl.res_why = "chunk state does not fit the 227 KB of shared memory of an SM"; return;
+  }
   R.nat_tpad = 0;
   pl.res_nat_rows = 0;
   if (C == 1 && !R.nat_smem && G == 1) {          // natives stay in global memory: read them coalesced
@@ -366,8 +373,8 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
   if ((size_t)((N + 31) / 32) * 8 > 200000) { pl.res_why = "n_beads too large for the localise bitmap"; return; }
   plan_resident2(tp, p, x, pl);
   if (getenv("SOP_DEBUG_PLAN"))
-    fprintf(stderr, "[sop plan] mode 3: C=%d chunk=%d lanes=%d block=%d halo_cap=%d cap_nb=%d cap_pl=%d nat_smem=%d pl_cap=%d smem=%d B\n",
-            R.C, R.chunk, pl.res_lanes, pl.res_block, R.halo_cap, pl.cap_nb, pl.cap_pl, R.nat_smem, R.pl_cap, R.smem_bytes);
+    fprintf(stderr, "[sop plan] mode 3: C=%d chunk=%d lanes=%d block=%d halo_cap=%d cap_nb=%d cap_pl=%d nat_smem=%d pl_cap=%d stream=%d smem=%d B\n",
+            R.C, R.chunk, pl.res_lanes, pl.res_block, R.halo_cap, pl.cap_nb, pl.cap_pl, R.nat_smem, R.pl_cap, R.stream, R.smem_bytes);
   pl.res_ok = true;
 }
 
@@ -474,7 +481,10 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
     plan_resident(tp, p, x, pl);
     if (pl.mode == 3 && !pl.res_ok) return fail(SOP_E_ARG, "mode 3 is not possible here: " + pl.res_why);
     // fallback: the streaming kernels; one launch per step once the chip is full (measured on cfg 4), else persistent
-    pl.mode = pl.res_ok ? 3 : (inst > 100000 ? 1 : 2);
+    // (auto does not pick the streamed variant of mode 3: on the 250,000-bead lattice it measured 76 us per step against 72 us
+    //  of the per-step launches -- DESIGN.md section 6; it runs when mode 3 is asked for)
+    const bool take3 = pl.res_ok && !(p->mode == 0 && pl.R.stream);
+    pl.mode = take3 ? 3 : (inst > 100000 ? 1 : 2);
   }
   pl.energy_blocks = (int)std::min<long long>(296, ((long long)N * 8 + 255) / 256);
 
@@ -529,6 +539,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
     pl.off_bondloc = take(multi ? I * pl.cap_b * 8 : 0);
     pl.off_xch = take(multi ? 2 * I * 32 : 0);
     pl.off_xchf = take(multi ? 2 * I * 32 : 0);
+    pl.off_nbglob = take(R.stream ? I * R.nb_si * 2 : 0);
     pl.off_plarr = take(pl.res2_ok ? I * pl.R2.cap_arr * 2 : 0);
     pl.off_plg = take(pl.res2_ok ? I * 2 : 0);
   }
@@ -748,6 +759,11 @@ const void *res2_kernel(bool comp, bool eps, int P) {
   return eps ? res2_fn_p<false, true>(P) : res2_fn_p<false, false>(P);
 }
 
+const void *resident_stream_kernel(int lanes, bool comp) {
+  if (lanes == 1) return comp ? (const void *)k_resident<1, true, true> : (const void *)k_resident<1, false, true>;
+  return comp ? (const void *)k_resident<2, true, true> : (const void *)k_resident<2, false, true>;
+}
+
 int resident_prepare(sop_handle *h) {
   const Plan &pl = h->plan;
   h->R = pl.R;
@@ -757,6 +773,7 @@ int resident_prepare(sop_handle *h) {
   R.pl_loc = (unsigned short *)(w + pl.off_plloc); R.nat_pack = (int2 *)(w + pl.off_natloc);
   R.bond_pack = (int2 *)(w + pl.off_bondloc); R.xch = (uint4 *)(w + pl.off_xch); R.xchf = (uint4 *)(w + pl.off_xchf);
   R.nat_T = nullptr;
+  R.nb_glob = (unsigned short *)(w + pl.off_nbglob);
   R.skew_chunk = 0; R.skew_period = 1; R.skew_ns = 0;
   if (const char *sk = getenv("SOP_TEST_SKEW")) {        // test hook "chunk,period,ns": one chunk runs late on some steps
     int a = 0, b = 1, c = 0;
@@ -768,7 +785,7 @@ int resident_prepare(sop_handle *h) {
     R.nat_T = (int2 *)(w + pl.off_natloc);
     k_transpose_nat<<<(h->S.N + 255) / 256, 256, 0, h->stream>>>(h->S, R);
   }
-  h->res_fn = resident_kernel(pl.res_lanes, pl.comp);
+  h->res_fn = R.stream ? resident_stream_kernel(pl.res_lanes, pl.comp) : resident_kernel(pl.res_lanes, pl.comp);
   CUDA_OK(cudaFuncSetAttribute(h->res_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, R.smem_bytes));
   const int loc_smem = ((h->S.N + 31) / 32) * 8 + R.chunk * 4;
   CUDA_OK(cudaFuncSetAttribute((const void *)k_localise, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(loc_smem, 1024)));

@@ -56,6 +56,9 @@ struct ResDev {
   int nat_cap;                // largest number of native entries of a chunk
   int pl_cap;                 // 16-bit entries of shared memory for the chunk's L1 rows (0: read them from global)
   int smem_bytes;
+  int stream;                 // the chunk state does not fit shared memory: only the coordinates (ONE time layer), tags, forces and
+                              // counters are resident; L2 rows, bonds, natives and L1 rows are streamed from global memory (L2)
+  unsigned short *nb_glob;    // [T*N][nb_si] L2 rows as slots (stream)
 };
 
 __device__ __forceinline__ float fast_rcp(float x) {
@@ -254,8 +257,12 @@ __device__ __forceinline__ int lower_bound_dev(const int *__restrict__ a, int n,
 //   (e) every nb_interval steps: fetch the whole halo of the new layer, Alg. 3 on the own rows (L1 rows resident in
 //        shared memory when they fit), new active set.
 // Coordinates and noise are double-buffered on the step parity.
+// STREAM (systems whose chunks do not fit shared memory, e.g. 250,000 beads on 148 SMs): one coordinate layer -- every read of
+// a step's coordinates lies before the block barrier that precedes the update, and a thread updates only its own bead, so the
+// update can be done in place --, and the lists live in global memory (L2-resident): rows are read coalesced, the partner
+// gathers stay in shared memory.
 // ------------------------------------------------------------------------------------------------
-template <int G, bool COMP>
+template <int G, bool COMP, bool STREAM = false>
 __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cur, unsigned long long step0, int n_steps,
                                                       int nb_interval, int filter_flags, uint32_t stamp0) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -266,14 +273,17 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   float4 *scarry = (float4 *)(smem_raw + R.off_carry);               // [chunk]      (COMP)
   uint32_t *stag = (uint32_t *)(smem_raw + R.off_tag);               // [chunk]
   float4 *sforce = (float4 *)(smem_raw + R.off_force);                // [chunk] internal force of this step
-  unsigned short *nb = (unsigned short *)(smem_raw + R.off_nb);      // L2 rows as slots, row stride nb_si
+  // (tc is blockIdx.x; the L2 rows of a streamed chunk start at its first bead instance)
+  unsigned short *nb = STREAM ? R.nb_glob + ((size_t)(blockIdx.x / R.C) * S.N + (size_t)(blockIdx.x % R.C) * R.chunk) * R.nb_si
+                              : (unsigned short *)(smem_raw + R.off_nb);      // L2 rows as slots, row stride nb_si
   unsigned short *cnt_s = (unsigned short *)(smem_raw + R.off_cnt);  // [chunk] L2 row counts
   unsigned short *plcnt_s = (unsigned short *)(smem_raw + R.off_plcnt);  // [chunk] L1 row counts
   int *plofs = (int *)(smem_raw + R.off_plofs);                      // [chunk + 1] L1 row starts in spl (even)
   unsigned short *spl = (unsigned short *)(smem_raw + R.off_pl);     // [pl_cap] L1 rows as slots, packed
   int *natq = (int *)(smem_raw + R.off_natq);                        // [chunk + 1] native table offsets
   int2 *snat = (int2 *)(smem_raw + R.off_nat);                       // [nat_cap]    (nat_smem)
-  int2 *sbond = (int2 *)(smem_raw + R.off_bond);                     // [chunk][cap_b]
+  int2 *sbond = STREAM ? R.bond_pack + ((size_t)(blockIdx.x / R.C) * S.N + (size_t)(blockIdx.x % R.C) * R.chunk) * S.cap_b
+                       : (int2 *)(smem_raw + R.off_bond);            // [chunk][cap_b]
   unsigned short *active = (unsigned short *)(smem_raw + R.off_active);
   uint32_t *bm = (uint32_t *)(smem_raw + R.off_bm), *sbm = (uint32_t *)(smem_raw + R.off_sbm);
   unsigned short *order = (unsigned short *)(smem_raw + R.off_order);     // own beads by descending native degree
@@ -320,7 +330,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   const int qbase = S.nat_ptr[b0];
   if (tid == 0) {      // a point 1e18 A away: its repulsion underflows to exactly zero (pads odd L2 rows)
     spos[SC - 1] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.f);
-    spos[2 * SC - 1] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.f);
+    if (!STREAM) spos[2 * SC - 1] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.f);
   }
   for (int i = tid; i < n_own; i += bd) {
     const float4 v = S.pos[cur][inst0 + b0 + i];
@@ -338,7 +348,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   }
   if (tid == 0) natq[n_own] = S.nat_ptr[b1];
   const int2 *bond_src = multi ? R.bond_pack + (inst0 + b0) * cap_b : S.bond_tab + (size_t)b0 * cap_b;
-  for (int e = tid; e < n_own * cap_b; e += bd) sbond[e] = bond_src[e];
+  if (!STREAM) for (int e = tid; e < n_own * cap_b; e += bd) sbond[e] = bond_src[e];
   const int2 *nat_glob = multi ? R.nat_pack + (size_t)t * R.nat_entries : S.nat_tab;
   const int n_nat = S.nat_ptr[b1] - qbase;
   if (R.nat_smem)
@@ -374,11 +384,13 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   __syncthreads();
   if (tid == 0) { int run = 0; for (int b = 0; b < 64; ++b) { const int c2 = hist[b]; hist[b] = run; run += c2; } }
   __syncthreads();
-  for (int i = tid; i < n_own; i += bd)           // one lane per bead: keep thread i on bead i (coalesced table reads)
-    order[G > 1 ? atomicAdd(&hist[63 - min(63, natq[i + 1] - natq[i])], 1) : i] = (unsigned short)i;
-  scan_counts(plcnt_s, plofs, true);
+  if (!STREAM) {
+    for (int i = tid; i < n_own; i += bd)           // one lane per bead: keep thread i on bead i (coalesced table reads)
+      order[G > 1 ? atomicAdd(&hist[63 - min(63, natq[i + 1] - natq[i])], 1) : i] = (unsigned short)i;
+    scan_counts(plcnt_s, plofs, true);
+  }
   __syncthreads();
-  const bool pl_in_smem = !R.implicit_l1 && R.pl_cap > 0 && plofs[n_own] <= R.pl_cap;
+  const bool pl_in_smem = !STREAM && !R.implicit_l1 && R.pl_cap > 0 && plofs[n_own] <= R.pl_cap;
   if (pl_in_smem) {
     for (int il = warp; il < n_own; il += nwarps) {
       const uint32_t *src = (const uint32_t *)(R.pl_loc + (inst0 + b0 + il) * S.cap_pl);
@@ -559,7 +571,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
       constexpr bool IN_SMEM = decltype(in_smem_t)::value;     // plain LDS when the rows are resident, else global loads
       for (int base = 0; base < n_own; base += fgroups) {
         const bool valid = base + frow < n_own;
-        const int il = order[valid ? base + frow : n_own - 1];      // dense beads together: similar L1 row lengths per warp
+        const int il = STREAM ? (valid ? base + frow : n_own - 1) : order[valid ? base + frow : n_own - 1];      // dense beads together: similar L1 row lengths per warp
         const int cnt1 = valid ? (int)plcnt_s[il] : 0;
         const int nw = (cnt1 + 1) >> 1;
         const float4 ri = P[il];
@@ -626,7 +638,8 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     }
     __syncthreads();
     // bitmap -> list: a warp per word, a lane per bit (the order of the list does not matter, only who polls what)
-    for (int w = warp; w < HW; w += nwarps) {
+    // (STREAM keeps the bitmap only: the list of a 9000-slot halo would not fit)
+    for (int w = warp; w < HW && !STREAM; w += nwarps) {
       const uint32_t m = bm[w];
       if (m) {
         int at = 0;
@@ -648,13 +661,22 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
   bool have_full = true;                     // the whole halo of the current layer is already in shared memory (prologue)
   for (int k = 0; k < n_steps; ++k) {
     const unsigned long long step = step0 + (unsigned long long)k;
-    float4 *pc = spos + (size_t)(k & 1) * SC, *pn = spos + (size_t)((k & 1) ^ 1) * SC;
+    float4 *pc = spos + (STREAM ? 0 : (size_t)(k & 1) * SC), *pn = spos + (STREAM ? 0 : (size_t)((k & 1) ^ 1) * SC);
     float4 *gc = sg + (size_t)(k & 1) * R.chunk, *gnx = sg + (size_t)((k & 1) ^ 1) * R.chunk;
     uint4 *const xc = (k & 1) ? xl1 : xl0, *const xn = (k & 1) ? xl0 : xl1;
     const uint32_t st_c = stamp0 + (uint32_t)k, st_n = st_c + 1u;
     const ExtStep ext = ext_step(S, step);          // fp64 conversions of the step number: before the waits, not after
     // (b) active halo of layer k: poll until the neighbours have published it
-    if (multi && !have_full) {
+    if (multi && !have_full && STREAM) {
+      for (int w = warp; w < HW; w += nwarps) {              // a warp per bitmap word, a lane per halo slot
+        if ((bm[w] >> wlane) & 1u) {
+          const int h = (w << 5) + wlane;
+          float4 v;
+          xch_wait(xc + 2 * (inst0 + hgid[h]), st_c, v, S.flags);
+          pc[n_own + h] = v;
+        }
+      }
+    } else if (multi && !have_full) {
       const int na = misc[0];
       for (int q = tid; q < na; q += bd) {
         const int slot = active[q];
@@ -671,7 +693,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
     // (d1) a4..a6: internal force, G lanes per bead (Alg. 2; no distance test in the loop, R3c)
     for (int base = 0; base < n_own; base += groups) {
       const bool valid = base + grp < n_own;
-      const int il = order[valid ? base + grp : n_own - 1];
+      const int il = STREAM ? (valid ? base + grp : n_own - 1) : order[valid ? base + grp : n_own - 1];
       const float4 ri = pc[il];
       float fx = 0.f, fy = 0.f, fz = 0.f;
       if (valid) {
@@ -706,15 +728,36 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
             fx += s * dx; fy += s * dy; fz += s * dz;
           }
         };
-        if (nat_eps) natives(std::true_type{}, std::false_type{});
+        if (STREAM && !nat_eps) {
+          // the table comes from global memory (L2): eight independent entry loads in flight, then their gathers
+          // (an entry past the end is the dummy slot with r0^2 = 0: its term is exactly zero)
+          const int q0 = natq[il];
+          for (int q = q0 + lane; q < q1; q += 8 * G) {
+            int2 en[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) en[u] = q + u * G < q1 ? __ldg(&natp[q + u * G]) : make_int2((int)DUMMY, 0);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+              const float4 rj = pc[en[u].x];
+              const float dx = ri.x - rj.x, dy = ri.y - rj.y, dz = ri.z - rj.z;
+              const float s = nat_s3(dx * dx + dy * dy + dz * dz, __int_as_float(en[u].y), K.eps12);
+              fx += s * dx; fy += s * dy; fz += s * dz;
+            }
+          }
+        }
+        else if (nat_eps) natives(std::true_type{}, std::false_type{});
         else if (R.nat_smem) natives(std::false_type{}, std::true_type{});
         else natives(std::false_type{}, std::false_type{});
         // a6: non-native repulsion   V = eps_r (sigma/r)^6; four slots per 8-byte word (rows are padded to a multiple
         // of four with the dummy slot): one index load, four gathers in flight
         const uint2 *row64 = (const uint2 *)(nb + (size_t)il * R.nb_si);
         const int n4 = ((int)cnt_s[il] + 3) >> 2;
+        uint2 wn = make_uint2(0u, 0u);
+        if (STREAM && lane < n4) wn = row64[lane];                  // (global memory: the next word is in flight while this one is used)
         for (int p = lane; p < n4; p += G) {
-          const uint2 w = row64[p];
+          uint2 w;
+          if (STREAM) { w = wn; if (p + G < n4) wn = row64[p + G]; }
+          else w = row64[p];
           const float4 ra = pc[w.x & 0xFFFFu], rb = pc[w.x >> 16], rc = pc[w.y & 0xFFFFu], rd = pc[w.y >> 16];
           const float ax = ri.x - ra.x, ay = ri.y - ra.y, az = ri.z - ra.z;
           const float bx = ri.x - rb.x, by = ri.y - rb.y, bz = ri.z - rb.z;
@@ -795,7 +838,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cu
 
   // ---- epilogue: the current layer, the carry and the L2 rows back to the canonical arrays
   __syncthreads();
-  const float4 *pf = spos + (size_t)(n_steps & 1) * SC;
+  const float4 *pf = spos + (STREAM ? 0 : (size_t)(n_steps & 1) * SC);
   for (int i = tid; i < n_own; i += bd) {
     S.pos[cur][inst0 + b0 + i] = pf[i];
     if (COMP) S.carry[inst0 + b0 + i] = scarry[i];

@@ -801,3 +801,30 @@ def test_pair_based_scheme_mode4(atomics):
 def test_pair_based_scheme_full_config0_and_3():
     full_check(0, mode=4)
     full_check(3, mode=4)
+
+
+# ---------------------------------------------------------------------------------------------- mode 3, streamed lists
+def test_mode3_streamed_lists_variant():
+    """Chunks whose state does not fit shared memory keep only the coordinates resident (one time layer, updated in place) and
+    stream L2 rows, bonds, natives and L1 rows from global memory.  SOP_TEST_STREAM forces that variant on small inputs:
+    forces, 230-step coordinates and lists against the oracle, bit-identical to itself however the run is split; the
+    250,000-bead lattice takes it when mode 3 is asked for."""
+    os.environ["SOP_TEST_STREAM"] = "1"
+    try:
+        w = gen.two_chains(150, 3, R_pl=20.0)
+        for var in (dict(chunk_beads=60, lanes_per_bead=1), dict(chunk_beads=75, lanes_per_bead=2, compensated=1)):
+            s = sop().from_workload(w, mode=3, **var)
+            o = sopo.from_workload(w)
+            f, fo = s.get_forces(), o.get_forces()
+            assert np.abs(f - fo).max() <= 1e-4 * np.abs(fo).max()
+            s.run(230); o.run(230)
+            xg = s.get_coords()
+            assert np.abs(xg - o.get_coords()).max() <= 3e-3
+            c1, i1, _ = s.get_lists(1); c2, i2, _ = s.get_lists(2)
+            oc, oi = o.filter(xg[0].astype(np.float64), c1, i1)
+            assert np.array_equal(c2, oc) and all(np.array_equal(i2[i, :c2[i]], oi[i, :oc[i]]) for i in range(w.n_beads))
+            b = sop().from_workload(w, mode=3, **var); b.run(100); b.run(130)
+            assert np.array_equal(b.get_coords(), xg)
+    finally:
+        del os.environ["SOP_TEST_STREAM"]
+    full_check(4, mode=3)
