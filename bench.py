@@ -279,7 +279,7 @@ def cpu_sample(w, T, n_steps):
 
 
 # oracle sample sizes (Langevin steps) giving roughly 10-20 s on 8 cores; multiples of pl_interval
-CPU_STEPS = {0: 20000, 1: 300, 2: 600, 3: 400, 4: 100}
+CPU_STEPS = {0: 40000, 1: 600, 2: 1200, 3: 1200, 4: 200}
 CPU_TRAJ = {1: 8}
 
 

@@ -313,6 +313,7 @@ void plan_resident(const sop_topology *tp, const sop_params *p, const std::vecto
     R.nat_cap = std::max(1, *std::max_element(per.begin(), per.end()));
   }
   R.nb_si = pl.cap_nb + 4;                       // rows padded to a multiple of four slots, 8-byte aligned
+  if (R.nb_si % 4 != 0) { pl.res_why = "internal: the L2 row stride must be a multiple of four slots"; return; }   // (cap_nb is)
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o = (o + bytes + 15) / 16 * 16; return (int)at; };
   auto carve = [&](bool nat_smem, int pl_cap, bool stream = false) {

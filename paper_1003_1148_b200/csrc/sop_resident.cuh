@@ -51,7 +51,8 @@ struct ResDev {
   // shared-memory carve-up (bytes from the start of dynamic shared memory), computed by the host
   int off_pos, off_g, off_carry, off_tag, off_force, off_nb, off_cnt, off_plcnt, off_plofs, off_pl, off_natq,
       off_nat, off_bond, off_active, off_bm, off_sbm, off_misc, off_order, off_hist;
-  int nb_si;                  // L2 row i starts at nb[i * nb_si] (an odd number of 32-bit words: conflict-free)
+  int nb_si;                  // L2 row i starts at nb[i * nb_si]; nb_si = cap_nb + 4 is a multiple of four 16-bit slots, so that every
+                              // row is 8-byte aligned (rows are read four slots per 8-byte word and padded with the dummy slot)
   int nat_smem;               // the chunk's native table is copied to shared memory (its nat_cap entries fit)
   int nat_cap;                // largest number of native entries of a chunk
   int pl_cap;                 // 16-bit entries of shared memory for the chunk's L1 rows (0: read them from global)
