@@ -576,6 +576,10 @@ void launch_step_g(sop_handle *h, bool forces) {
   const unsigned grid = (unsigned)((threads + block - 1) / block);
   const unsigned long long step = (unsigned long long)h->step;
   if (forces) k_step<G, false, true><<<grid, block, 0, h->stream>>>(S, h->cur, step);
+  else if (block <= 256) {
+    if (h->plan.comp) k_step<G, true, false, true><<<grid, block, 0, h->stream>>>(S, h->cur, step);
+    else k_step<G, false, false, true><<<grid, block, 0, h->stream>>>(S, h->cur, step);
+  }
   else if (h->plan.comp) k_step<G, true, false><<<grid, block, 0, h->stream>>>(S, h->cur, step);
   else k_step<G, false, false><<<grid, block, 0, h->stream>>>(S, h->cur, step);
   h->launches++;

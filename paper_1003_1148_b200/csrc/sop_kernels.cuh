@@ -9,8 +9,10 @@ namespace sop {
 // organisation), G lanes per bead.  FORCES = true: the non-fused instantiation that writes the
 // deterministic force instead of moving the bead (sop_get_forces).
 // ------------------------------------------------------------------------------------------------
-template <int G, bool COMP, bool FORCES>
-__global__ void __launch_bounds__(1024) k_step(SysDev S, int cur, unsigned long long step) {
+// DENSE: blocks of <= 256 threads compiled for 32 registers (a few spilled words), so that 2048 threads are resident per SM:
+// the streaming step waits on dependent index -> coordinate gathers, and occupancy is what hides them (cfg 4: 44 -> 38 us).
+template <int G, bool COMP, bool FORCES, bool DENSE = false>
+__global__ void __launch_bounds__(DENSE ? 256 : 1024, DENSE ? 8 : 1) k_step(SysDev S, int cur, unsigned long long step) {
   const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int g = (int)(gid / G);
   const int lane = (int)(gid % G);
@@ -109,7 +111,9 @@ __global__ void k_taus_seed(SysDev S, int cur) {
 }
 
 // a3: L2 neighbor-list filter (Alg. 3), one warp per bead instance.
-__global__ void __launch_bounds__(256) k_filter(SysDev S, int cur) {
+// 32 registers (two small spills) so that 2048 threads are resident: the kernel waits on its gathers, and the extra warps
+// hide them (cfg 4: 164 -> 148 us; larger blocks or 8 lanes per row with 64-bit masks measured slower)
+__global__ void __launch_bounds__(256, 8) k_filter(SysDev S, int cur) {
   const int w = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
   const int lane = threadIdx.x & 31;
   if (w >= S.n_inst) return;
