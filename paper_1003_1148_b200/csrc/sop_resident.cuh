@@ -263,8 +263,8 @@ __device__ __forceinline__ int lower_bound_dev(const int *__restrict__ a, int n,
 // update can be done in place --, and the lists live in global memory (L2-resident): rows are read coalesced, the partner
 // gathers stay in shared memory.
 // ------------------------------------------------------------------------------------------------
-template <int G, bool COMP, bool STREAM = false>
-__global__ void __launch_bounds__(1024, 1) k_resident(SysDev S, ResDev R, int cur, unsigned long long step0, int n_steps,
+template <int G, bool COMP, bool STREAM = false, int MAXT = 1024>
+__global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cur, unsigned long long step0, int n_steps,
                                                       int nb_interval, int filter_flags, uint32_t stamp0) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const bool filter_last = filter_flags & 1, filter_first = filter_flags & 2;
