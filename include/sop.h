@@ -129,6 +129,21 @@ int sop_set_coords(sop_handle *, const float *xyz /*HOST [T][N][3]*/);   /* rebu
 /* Eq. (1) term by term + external terms, per trajectory: fene, native, rep (over the current
  * L2, each pair once), pull, tip, total.  fp32 pair terms, fp64 accumulation. */
 int sop_get_energies(sop_handle *, double *e_out /*HOST [T][6]*/);
+/* The same six energies for callers that may not allocate device memory or wait for the host (code under CUDA graph
+ * capture, tight serving loops): sop_energies_noalloc enqueues the a10 reduction on the handle's stream with its per-block
+ * partial sums in a file-scope static __device__ array of SOP_NOALLOC_SCRATCH_BYTES inside the library (every GPU that
+ * loads the library holds it until exit) and writes {fene, native, rep, pull, tip, total} per trajectory to the caller's
+ * DEVICE array.  It calls no cudaMalloc / cudaFree / allocating routine, copies nothing to the host and does not
+ * synchronise: the result is valid once the stream has reached it (sop_sync); device-side conditions (FENE overstretch ...)
+ * are reported by the next synchronising call, as for sop_run.  Values are bit-identical to sop_get_energies.
+ * The scratch is shared by every handle and every call on a device and keeps the last call's contents (nothing in it has
+ * to start at zero: every block overwrites its own partial sums before they are read): calls that overlap on the GPU --
+ * two handles on different streams -- race and must be ordered by the caller.
+ * Errors: SOP_E_ARG for a null argument or when n_traj x reduction blocks x 5 doubles exceed SOP_NOALLOC_SCRATCH_BYTES
+ * (the message states both sizes; use sop_get_energies then); SOP_E_CUDA when the scratch address cannot be resolved
+ * or a launch fails. */
+#define SOP_NOALLOC_SCRATCH_BYTES (1u << 20)
+int sop_energies_noalloc(sop_handle *, double *d_e_out /*DEVICE [T][6]*/);
 /* Observables of the paper's applications, per trajectory, reduced on the device (PAPER.md:261 force-extension curves
  * f(R); :312-314 force-indentation): o[0] = radius of gyration, o[1] = end-to-end distance X between the first fixed
  * bead (else bead 0) and the first pulled bead (else bead N-1), o[2] = cantilever force summed over the pulled beads

@@ -886,6 +886,47 @@ int record_sample(sop_handle *h) {
   return check_launch(h, "observable sample");
 }
 
+// ------------------------------------------------------------------------------------------------
+// sop_energies_noalloc (include/sop.h): the a10 reduction with its scratch in a file-scope static __device__ array, for
+// callers that may not allocate.  In HOST code the name g_noalloc_scratch is a host-side stand-in, not a device address:
+// the address a kernel may use comes from cudaGetSymbolAddress, resolved once per device with that device current.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_noalloc_scratch[SOP_NOALLOC_SCRATCH_BYTES / sizeof(double)];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+double *g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};          // device address of the array on each device, once resolved
+
+// block partials -> {fene, native, rep, pull, tip, total} per trajectory: the blocks in order (as k_energy_final), the total
+// as sop_get_energies forms it on the host ((((e0 + e1) + e2) + e3) + e4 in fp64), so that the two paths agree bit for bit
+__global__ void k_energy_final_total(int T, int nblk, const double *partial, double *e_out) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= T) return;
+  double e[5];
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    double v = 0;
+    for (int b = 0; b < nblk; ++b) v += partial[((size_t)t * nblk + b) * 5 + k];
+    e[k] = v;
+    e_out[(size_t)t * 6 + k] = v;
+  }
+  e_out[(size_t)t * 6 + 5] = e[0] + e[1] + e[2] + e[3] + e[4];
+}
+
+int noalloc_scratch(sop_handle *h, double **out) {
+  int dev = -1;
+  CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(SOP_E_CUDA, "sop_energies_noalloc: device ordinal out of range", h);
+  if (!g_noalloc_ptr[dev]) {
+    double *p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void **)&p, g_noalloc_scratch);
+    if (e != cudaSuccess || !p)
+      return fail(SOP_E_CUDA, std::string("sop_energies_noalloc: cudaGetSymbolAddress: ") + cudaGetErrorString(e), h);
+    g_noalloc_ptr[dev] = p;       // (two threads racing here store the same address)
+  }
+  *out = g_noalloc_ptr[dev];
+  return SOP_OK;
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -1300,6 +1341,24 @@ int sop_get_energies(sop_handle *h, double *e_out) {
     e[5] = e[0] + e[1] + e[2] + e[3] + e[4];
   }
   return rc;
+}
+
+int sop_energies_noalloc(sop_handle *h, double *d_e_out) {
+  if (!h || !d_e_out) return fail(SOP_E_ARG, "null argument", h);
+  const SysDev &S = h->S;
+  const size_t need = (size_t)S.T * (size_t)h->plan.energy_blocks * 5 * sizeof(double);
+  if (need > (size_t)SOP_NOALLOC_SCRATCH_BYTES)
+    return fail(SOP_E_ARG, "sop_energies_noalloc: " + std::to_string(S.T) + " trajectories x " + std::to_string(h->plan.energy_blocks) +
+                " reduction blocks need " + std::to_string(need) + " bytes of scratch, the static scratch holds " +
+                std::to_string((size_t)SOP_NOALLOC_SCRATCH_BYTES) + " (use sop_get_energies)", h);
+  double *partial = nullptr;
+  int rc = noalloc_scratch(h, &partial);
+  if (rc) return rc;
+  dim3 grid((unsigned)h->plan.energy_blocks, (unsigned)S.T);
+  k_energy<<<grid, 256, 0, h->stream>>>(S, h->cur, (unsigned long long)h->step, partial);
+  k_energy_final_total<<<(S.T + 127) / 128, 128, 0, h->stream>>>(S.T, h->plan.energy_blocks, partial, d_e_out);
+  h->launches += 2;
+  return check_launch(h, "energy (no-alloc)");
 }
 
 int sop_replica_exchange(sop_handle *h, int32_t parity, uint64_t sweep, int32_t *accepted_out) {

@@ -14,10 +14,13 @@ _lib = None
 STATUS = {0: "SOP_OK", -1: "SOP_E_ARG", -2: "SOP_E_CUDA", -3: "SOP_E_LIST_OVERFLOW", -4: "SOP_E_FENE",
           -5: "SOP_E_NONFINITE"}
 
+NOALLOC_SCRATCH_BYTES = 1 << 20      # SOP_NOALLOC_SCRATCH_BYTES of include/sop.h
+
 SYMBOLS = ["sop_query_workspace", "sop_create", "sop_destroy", "sop_run", "sop_sync", "sop_get_coords",
            "sop_set_coords", "sop_get_energies", "sop_get_observables", "sop_get_forces", "sop_get_lists", "sop_get_step", "sop_set_step",
            "sop_device_coords", "sop_get_config", "sop_set_profiling", "sop_get_profile", "sop_last_error",
-           "sop_set_observable_stride", "sop_get_observable_series", "sop_replica_exchange", "sop_get_temperatures"]
+           "sop_set_observable_stride", "sop_get_observable_series", "sop_replica_exchange", "sop_get_temperatures",
+           "sop_energies_noalloc"]
 
 
 class _Topology(C.Structure):
@@ -71,6 +74,7 @@ def lib():
         L.sop_get_coords.argtypes = [vp, vp]
         L.sop_set_coords.argtypes = [vp, vp]
         L.sop_get_energies.argtypes = [vp, vp]
+        L.sop_energies_noalloc.argtypes = [vp, vp]
         L.sop_get_forces.argtypes = [vp, vp]
         L.sop_get_observables.argtypes = [vp, vp]
         L.sop_set_observable_stride.argtypes = [vp, i32]
@@ -201,6 +205,15 @@ class Sop:
         self._chk(lib().sop_get_energies(self._h, out.ctypes.data), "sop_get_energies")
         return out
 
+    def energies_noalloc(self, d_out):
+        """sop_energies_noalloc: the six energies into the caller's DEVICE tensor [T][6] float64; nothing is allocated, nothing
+        copied to the host, no synchronisation (the result is valid after sync()).  Scratch: a static device array of
+        NOALLOC_SCRATCH_BYTES shared by every call on the device."""
+        if not (d_out.is_cuda and d_out.is_contiguous() and d_out.dtype.itemsize == 8 and d_out.numel() >= self.T * 6):
+            raise ValueError("d_out must be a contiguous CUDA float64 tensor of at least T * 6 elements")
+        self._chk(lib().sop_energies_noalloc(self._h, d_out.data_ptr()), "sop_energies_noalloc")
+        return d_out
+
     # -- hooks
     def get_observables(self):
         """[T][4] float64: Rg, end-to-end distance, cantilever force, tip force (reduced on the device)."""
@@ -296,6 +309,7 @@ def sop_sync(h): return h.sync()
 def sop_get_coords(h): return h.get_coords()
 def sop_set_coords(h, xyz): return h.set_coords(xyz)
 def sop_get_energies(h): return h.get_energies()
+def sop_energies_noalloc(h, d_out): return h.energies_noalloc(d_out)
 def sop_get_forces(h): return h.get_forces()
 def sop_get_observables(h): return h.get_observables()
 def sop_replica_exchange(h, parity, sweep): return h.replica_exchange(parity, sweep)
