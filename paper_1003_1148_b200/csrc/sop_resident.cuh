@@ -523,6 +523,16 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
         }
       }
       __syncthreads();
+      // cell-sorted copy of the coordinates (.w = slot) in the force buffer, which is dead between the update and the next
+      // pair phase: the row scan below then streams its candidates without a dependent index load per candidate
+      float4 *gpos = sforce;
+      for (int q = tid; q < n_own; q += bd) {
+        const int j = gbead[q];
+        float4 r = P[j];
+        r.w = __int_as_float(j);
+        gpos[q] = r;
+      }
+      __syncthreads();
       // one thread per row: with a whole trajectory in the chunk there are about as many rows as threads, and a
       // private counter compacts without ballots (12x fewer warp instructions than a warp per row, measured)
       for (int il = tid; il < n_own; il += bd) {
@@ -535,9 +545,11 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
           for (int y = max(cy - 1, 0); y <= min(cy + 1, ny - 1); ++y) {
             const int c0 = (z * ny + y) * nx + max(cx - 1, 0), c1 = (z * ny + y) * nx + min(cx + 1, nx - 1);
             const int e0 = gstart[c1 + 1];
+#pragma unroll 4
             for (int q = gstart[c0]; q < e0; ++q) {
-              const int j = gbead[q];
-              if (j != il && pred32(ri, P[j], S.R_nb2)) {
+              const float4 rj = gpos[q];
+              const int j = __float_as_int(rj.w);
+              if (j != il && pred32(ri, rj, S.R_nb2)) {
                 if (n < R.nb_si) row[n] = (unsigned short)j;
                 ++n;
               }
@@ -745,6 +757,26 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
             int2 en[8];
 #pragma unroll
             for (int u = 0; u < 8; ++u) en[u] = q + u * G < q1 ? __ldg(&natp[q + u * G]) : make_int2((int)DUMMY, 0);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+              const float4 rj = pc[en[u].x];
+              const float dx = ri.x - rj.x, dy = ri.y - rj.y, dz = ri.z - rj.z;
+              const float s = nat_s3(dx * dx + dy * dy + dz * dz, __int_as_float(en[u].y), K.eps12);
+              fx += s * dx; fy += s * dy; fz += s * dz;
+            }
+          }
+        }
+        else if (!nat_eps && R.nat_T) {
+          // one-chunk trajectories with one lane per bead (cfg 1): the transposed table is read coalesced from L2, eight
+          // independent entry loads in flight instead of one L2 round trip per native contact (same order of summation;
+          // an entry past the end is the dummy slot with r0^2 = 0: its term is exactly zero)
+          const int nq = q1 - natq[il];
+          const int tpad = R.nat_tpad;                      // (rows x tpad entries fit 32 bits: N <= 65535 slots per chunk)
+          for (int r = 0; r < nq; r += 8) {
+            int2 en[8];
+            const int2 *np = R.nat_T + (r * tpad + il);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) en[u] = r + u < nq ? __ldg(np + u * tpad) : make_int2((int)DUMMY, 0);
 #pragma unroll
             for (int u = 0; u < 8; ++u) {
               const float4 rj = pc[en[u].x];
