@@ -177,8 +177,10 @@ int sop_set_step(sop_handle *, int64_t step);       /* with sop_set_coords: exac
  * perm_out (HOST [N], may be NULL) receives the caller index of each internal slot. */
 int sop_device_coords(sop_handle *, void **d_float4_out, int32_t *perm_out);
 /* What the auto settings resolved to: lanes_per_bead, block_size, compensated(0/1), mode(1/2/3), reorder(0/1),
- * cap_nb, cap_pl, kernel launches issued so far (lo, hi), resident_variant in use (0 when the trajectory is one chunk). */
-int sop_get_config(sop_handle *, int32_t out[10]);
+ * cap_nb, cap_pl, kernel launches issued so far (lo, hi), resident_variant in use (0 when the trajectory is one chunk),
+ * steps per time slice of the most recent SLICED mode-3 launch (0: none so far; many one-chunk trajectories,
+ * PAPER.md:292), reserved. */
+int sop_get_config(sop_handle *, int32_t out[12]);
 /* Kernel timing for the bench (CUDA events on the handle's stream around groups of launches of one kind).
  * sop_get_profile synchronises, fills out[0..2] = ms spent in {step kernels, L2 filter kernels, L1 build kernels},
  * out[3..5] = number of timed spans of each kind, out[6] = Langevin steps covered by the step spans, and resets. */

@@ -42,7 +42,7 @@ struct Plan {                     // everything that depends only on (topology, 
   std::string res_why;
   int res_lanes = 1, res_block = 1024, res_nat_rows = 0;
   ResDev R;
-  size_t off_nhalo, off_hgid, off_plloc, off_natloc, off_bondloc, off_xch, off_xchf, off_nbglob;
+  size_t off_nhalo, off_hgid, off_plloc, off_natloc, off_bondloc, off_xch, off_xchf, off_nbglob, off_slice;
   // mode 3, several chunks per trajectory: the second resident kernel (sop_resident2.cuh) when its plan fits
   bool res2_ok = false;
   int res2_block = 0;
@@ -87,6 +87,7 @@ struct sop_handle {
   int obs_a = 0, obs_b = 0;       // internal indices of the two ends of the end-to-end distance
   const void *res_fn = nullptr;
   uint32_t res_launch_id = 0;
+  int last_slice_len = 0;              // steps per time slice of the most recent sliced mode-3 launch (0: none so far)
   std::vector<uint32_t> tag;      // [N] host copy of the coordinate tags (internal order)
   float4 *stage = nullptr;        // pinned host staging buffer [T][N] for coordinate transfers
   // optional kernel timing (sop_set_profiling): event pairs around groups of launches of one kind
@@ -541,6 +542,7 @@ int make_plan(const sop_topology *tp, const float *xyz, const sop_params *p, int
     pl.off_xch = take(multi ? 2 * I * 32 : 0);
     pl.off_xchf = take(multi ? 2 * I * 32 : 0);
     pl.off_nbglob = take(R.stream ? I * R.nb_si * 2 : 0);
+    pl.off_slice = take(R.C == 1 ? ((size_t)T + 1) * 4 : 0);        // ticket counter + done[T] of a sliced launch
     pl.off_plarr = take(pl.res2_ok ? I * pl.R2.cap_arr * 2 : 0);
     pl.off_plg = take(pl.res2_ok ? I * 2 : 0);
   }
@@ -754,6 +756,9 @@ const void *resident_fn(bool comp, int block) {
 }
 
 const void *resident_kernel(int lanes, bool comp, int block) {
+#ifdef SOP_DEV_MIN      // development builds only (compile time): the instantiations cfg 1 / cfg 2 / cfg 3 take
+  return lanes == 1 ? resident_fn<1>(comp, block) : lanes == 2 ? resident_fn<2>(comp, block) : resident_fn<4>(comp, block);
+#else
   switch (lanes) {
     case 1: return resident_fn<1>(comp, block);
     case 2: return resident_fn<2>(comp, block);
@@ -762,6 +767,7 @@ const void *resident_kernel(int lanes, bool comp, int block) {
     case 16: return resident_fn<16>(comp, block);
     default: return resident_fn<32>(comp, block);
   }
+#endif
 }
 
 template <bool COMP, bool EPS>
@@ -769,8 +775,12 @@ const void *res2_fn_p(int P) {
   return P == 1 ? (const void *)k_res2<COMP, EPS, 1> : (const void *)k_res2<COMP, EPS, 2>;
 }
 const void *res2_kernel(bool comp, bool eps, int P) {
+#ifdef SOP_DEV_MIN
+  return nullptr;
+#else
   if (comp) return eps ? res2_fn_p<true, true>(P) : res2_fn_p<true, false>(P);
   return eps ? res2_fn_p<false, true>(P) : res2_fn_p<false, false>(P);
+#endif
 }
 
 const void *resident_stream_kernel(int lanes, bool comp) {
@@ -788,6 +798,7 @@ int resident_prepare(sop_handle *h) {
   R.bond_pack = (int2 *)(w + pl.off_bondloc); R.xch = (uint4 *)(w + pl.off_xch); R.xchf = (uint4 *)(w + pl.off_xchf);
   R.nat_T = nullptr;
   R.nb_glob = (unsigned short *)(w + pl.off_nbglob);
+  R.slice_len = 0; R.ticket = (int *)(w + pl.off_slice); R.done = R.ticket + 1;
   R.skew_chunk = 0; R.skew_period = 1; R.skew_ns = 0;
   if (const char *sk = getenv("SOP_TEST_SKEW")) {        // test hook "chunk,period,ns": one chunk runs late on some steps
     int a = 0, b = 1, c = 0;
@@ -835,8 +846,31 @@ int resident_launch(sop_handle *h, int n, bool filter_last, bool filter_first) {
   int nb = h->prm.nb_interval, fl = (filter_last ? 1 : 0) | (filter_first ? 2 : 0);
   h->res_launch_id++;
   uint32_t stamp0 = ((h->res_launch_id & 0xFFFu) << 20) | 1u;     // never 0, never the previous launch's stamps
+  // One chunk per trajectory and more trajectories than SMs (the many-runs batch): T CTAs of one SM each
+  // would run in ceil(T / SMs) waves with the last one partly empty (256 on 148: 14 % of the machine idle).  The launch is cut
+  // into time slices instead -- one CTA per (slice, trajectory), handed out slice-major by a ticket, a trajectory's slices
+  // chained through `done` -- so every SM is busy until the last wave of slices.  A slice is what a separate launch of
+  // slice_len steps would be (same prologue / epilogue, same bits); slice_len is a multiple of nb_interval.
+  unsigned n_cta = (unsigned)(S.T * R.C);
+  if (R.C == 1 && !h->plan.res2_ok && !R.stream && S.T > device_sm_count() && !getenv("SOP_NO_SLICES")) {
+    const int sms = device_sm_count();
+    long long best_cost = 0; int best_len = 0;
+    for (int len = 2 * nb; len < n; len += nb) {
+      const long long slices = (n + len - 1) / len;
+      const long long waves = (slices * S.T + sms - 1) / sms;
+      const long long cost = waves * (2 * len + 3);           // (a slice costs about 1.5 steps of prologue + epilogue)
+      if (!best_len || cost < best_cost) { best_cost = cost; best_len = len; }
+    }
+    const long long plain = (long long)((S.T + sms - 1) / sms) * (2 * n + 3);
+    if (best_len && best_cost * 100 < plain * 97) {
+      R.slice_len = best_len;
+      h->last_slice_len = best_len;
+      n_cta = (unsigned)(((n + best_len - 1) / best_len) * S.T);
+      CUDA_OK(cudaMemsetAsync(R.ticket, 0, ((size_t)S.T + 1) * 4, h->stream));
+    }
+  }
   void *args[] = {&S, &R, &cur, &step0, &n, &nb, &fl, &stamp0};
-  const dim3 grid((unsigned)(S.T * R.C)), block((unsigned)h->plan.res_block);
+  const dim3 grid(n_cta), block((unsigned)h->plan.res_block);
   if (h->plan.res2_ok) {
     Res2Dev Q = h->R2;
     void *args2[] = {&S, &R, &Q, &cur, &step0, &n, &nb, &fl, &stamp0};
@@ -1475,13 +1509,14 @@ extern "C" int sop_debug_phase_clocks(sop_handle *h, float *out, int n_float4) {
 }
 #endif
 
-int sop_get_config(sop_handle *h, int32_t out[10]) {
+int sop_get_config(sop_handle *h, int32_t out[12]) {
   if (!h || !out) return fail(SOP_E_ARG, "null argument", h);
   out[0] = h->plan.mode == 3 ? h->plan.res_lanes : h->plan.lanes; out[1] = h->plan.mode == 3 ? h->plan.res_block : h->plan.block; out[2] = h->plan.comp; out[3] = h->plan.mode;
   out[4] = h->plan.reorder; out[5] = h->plan.cap_nb; out[6] = h->plan.cap_pl;
   out[7] = (int32_t)(h->launches & 0xFFFFFFFFu); out[8] = (int32_t)(h->launches >> 32);
   out[9] = h->plan.mode == 3 && h->R.C > 1 ? (h->plan.res2_ok ? 2 : 1) : 0;
   if (out[9] == 2) { out[0] = R2_GS; out[1] = h->plan.res2_block; }
+  out[10] = h->last_slice_len; out[11] = 0;
   return SOP_OK;
 }
 

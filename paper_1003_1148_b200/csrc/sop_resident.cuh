@@ -47,6 +47,11 @@ struct ResDev {
   uint4 *xch;                 // [2][T*N][2]  step layers: one 32-byte slot {x|stamp, y|stamp, z|stamp, -} per bead and step parity
   uint4 *xchf;                // [2][T*N][2]  filter layers: the coordinates of the steps on which L2 is re-filtered (read by the
                               //              WHOLE halo), alternating with the parity of step / nb_interval
+  // one chunk per trajectory and more trajectories than SMs: a launch is cut into time slices of slice_len steps, one CTA per
+  // (slice, trajectory), handed out slice-major by a ticket counter; a CTA waits until its trajectory's previous slice has
+  // signalled `done`, so that the grid fills every SM all the time instead of running T CTAs in ceil(T / SMs) waves
+  int slice_len;              // 0: one CTA per chunk for the whole launch
+  int *ticket, *done;         // [1], [T]  (zeroed by the host before a sliced launch)
   int skew_chunk, skew_period, skew_ns;   // test hook: chunk skew_chunk sleeps skew_ns before publishing on steps % skew_period == 0
   // shared-memory carve-up (bytes from the start of dynamic shared memory), computed by the host
   int off_pos, off_g, off_carry, off_tag, off_force, off_nb, off_cnt, off_plcnt, off_plofs, off_pl, off_natq,
@@ -267,7 +272,6 @@ template <int G, bool COMP, bool STREAM = false, int MAXT = 1024>
 __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cur, unsigned long long step0, int n_steps,
                                                       int nb_interval, int filter_flags, uint32_t stamp0) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const bool filter_last = filter_flags & 1, filter_first = filter_flags & 2;
   const int SC = R.chunk + R.halo_cap + 1;                           // + the dummy slot (last)
   float4 *spos = (float4 *)(smem_raw + R.off_pos);                   // [2][SC]
   float4 *sg = (float4 *)(smem_raw + R.off_g);                       // [2][chunk]
@@ -291,7 +295,34 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
   int *hist = (int *)(smem_raw + R.off_hist);                              // [64] scratch of that counting sort
   int *misc = (int *)(smem_raw + R.off_misc);                        // [0] active halo slots, [2..7] bounding box of the in-kernel grid
 
-  const int tc = blockIdx.x, t = tc / R.C, c = tc - t * R.C;
+  int tc = blockIdx.x, slice = 0;
+  if (!STREAM && R.slice_len > 0) {
+    // sliced launch (C == 1): ticket -> (slice, trajectory); tickets are handed out in order, so the CTA that owns this
+    // trajectory's previous slice took its ticket earlier and is running or done -- the wait below cannot deadlock
+    __shared__ int s_ticket;
+    if (threadIdx.x == 0) s_ticket = atomicAdd(R.ticket, 1);
+    __syncthreads();
+    const int n_tc = S.T * R.C, n_total = n_steps;
+    slice = s_ticket / n_tc; tc = s_ticket - slice * n_tc;
+    step0 += (unsigned long long)slice * (unsigned long long)R.slice_len;
+    n_steps = min(R.slice_len, n_total - slice * R.slice_len);
+    const bool last = (slice + 1) * R.slice_len >= n_total;
+    // (slice_len is a multiple of nb_interval: the filter due at the end of an inner slice runs inside it)
+    filter_flags = (last ? (filter_flags & 1) : 1) | (slice == 0 ? (filter_flags & 2) : 0);
+    if (slice > 0) {
+      if (threadIdx.x == 0) {
+        int seen;
+        do {
+          asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(R.done + tc) : "memory");
+          if (seen < slice) __nanosleep(200);
+        } while (seen < slice);
+      }
+      __syncthreads();
+      __threadfence();                         // every thread reads what the previous slice wrote (no stale L1 lines)
+    }
+  }
+  const bool filter_last = filter_flags & 1, filter_first = filter_flags & 2;
+  const int t = tc / R.C, c = tc - t * R.C;
   const int b0 = c * R.chunk, b1 = min(S.N, b0 + R.chunk), n_own = b1 - b0;
   const bool multi = R.C > 1;
   const int n_halo = multi ? R.n_halo[tc] : 0;
@@ -895,6 +926,10 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
     if (wlane == 0) S.nb_cnt[g] = cnt;
   }
   if (flag) atomicOr(S.flags, flag);
+  if (!STREAM && R.slice_len > 0) {            // this trajectory's next slice may start: release what every thread wrote
+    __syncthreads();
+    if (tid == 0) { __threadfence(); asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(R.done + tc), "r"(slice + 1) : "memory"); }
+  }
 }
 
 }  // namespace sop

@@ -270,12 +270,13 @@ class Sop:
         self._chk(lib().sop_set_step(self._h, int(v)), "sop_set_step")
 
     def config(self):
-        out = np.zeros(10, np.int32)
+        out = np.zeros(12, np.int32)
         self._chk(lib().sop_get_config(self._h, out.ctypes.data), "sop_get_config")
         names = ["lanes_per_bead", "block_size", "compensated", "mode", "reorder", "cap_nb", "cap_pl"]
         d = {k: int(v) for k, v in zip(names, out[:7])}
         d["launches"] = int(np.uint32(out[7])) | (int(np.uint32(out[8])) << 32)
         d["resident_variant"] = int(out[9])
+        d["slice_len"] = int(out[10])
         return d
 
     def set_profiling(self, on=True):

@@ -316,6 +316,33 @@ def test_full_config1_batch(mode):
     assert s.config()["mode"] == mode
 
 
+@pytest.mark.parametrize("R_pl", [float("inf"), 20.0], ids=["static_l1", "finite_l1"])
+def test_many_trajectories_sliced_launch_is_bit_identical(R_pl):
+    """More one-chunk trajectories than SMs: a mode-3 launch is cut into time slices (one CTA per slice and trajectory, handed
+    out by a ticket, chained per trajectory) so that no SM idles through a partly empty last wave.  A slice is what a separate
+    launch would be, so coordinates, lists and energies must be bit-identical to the unsliced launch (SOP_NO_SLICES), also
+    when the run is split; sample trajectories against the oracle."""
+    w = gen.globule(96, 77, R_pl=R_pl)
+    T = 160
+    a = sop().from_workload(w, n_traj=T, mode=3); a.run(230)
+    assert a.config()["mode"] == 3 and a.config()["slice_len"] > 0
+    os.environ["SOP_NO_SLICES"] = "1"
+    try:
+        b = sop().from_workload(w, n_traj=T, mode=3); b.run(230)
+        assert b.config()["slice_len"] == 0
+    finally:
+        del os.environ["SOP_NO_SLICES"]
+    c = sop().from_workload(w, n_traj=T, mode=3); c.run(95); c.run(135)
+    xa = a.get_coords()
+    assert np.array_equal(xa, b.get_coords()) and np.array_equal(xa, c.get_coords())
+    assert np.array_equal(a.get_energies(), b.get_energies())
+    for t in (0, 97, T - 1):
+        ca, ia, ata = a.get_lists(2, t); cb, ib, atb = b.get_lists(2, t)
+        assert rows_equal(ca, ia, cb, ib) and ata == atb == 230
+    o = sopo.from_workload(w, n_traj=T); o.run(230)
+    assert np.abs(xa - o.get_coords()).max() <= 3e-3           # (230 steps: DESIGN.md section 8, "beyond 100 steps")
+
+
 def test_full_config1_batch_finite_pair_list():
     w = gen.config1(R_pl=20.0)
     T = 16
