@@ -380,7 +380,7 @@ def main():
                 if k == args.config:
                     continue
                 wk = gen.make_config(k)
-                blk = 1000 if wk.n_beads * wk.n_traj < 100000 else 200
+                blk = 1000 if wk.n_beads * wk.n_traj < 100000 or k == 1 else 200     # (cfg 4 launches per step: 200 suffice)
                 r = measure(wk, wk.n_traj, 0, blk, 3, 3, e2e=False, overrides=over)
                 sweep[wk.name] = {"value": r["value"], "us_per_langevin_step": r["us_per_langevin_step"],
                                   "step_kernel_us": r.get("step_kernel", {}).get("us_per_langevin_step"),

@@ -858,10 +858,10 @@ int resident_launch(sop_handle *h, int n, bool filter_last, bool filter_first) {
     for (int len = 2 * nb; len < n; len += nb) {
       const long long slices = (n + len - 1) / len;
       const long long waves = (slices * S.T + sms - 1) / sms;
-      const long long cost = waves * (2 * len + 3);           // (a slice costs about 1.5 steps of prologue + epilogue)
+      const long long cost = waves * (2 * len + 7);           // (a slice costs about 3.5 steps of prologue + epilogue: measured)
       if (!best_len || cost < best_cost) { best_cost = cost; best_len = len; }
     }
-    const long long plain = (long long)((S.T + sms - 1) / sms) * (2 * n + 3);
+    const long long plain = (long long)((S.T + sms - 1) / sms) * (2 * n + 7);
     if (best_len && best_cost * 100 < plain * 97) {
       R.slice_len = best_len;
       h->last_slice_len = best_len;
