@@ -87,6 +87,7 @@ struct sop_handle {
   int obs_a = 0, obs_b = 0;       // internal indices of the two ends of the end-to-end distance
   const void *res_fn = nullptr;
   uint32_t res_launch_id = 0;
+  int res_resident_ctas = 148;
   int last_slice_len = 0;              // steps per time slice of the most recent sliced mode-3 launch (0: none so far)
   std::vector<uint32_t> tag;      // [N] host copy of the coordinate tags (internal order)
   float4 *stage = nullptr;        // pinned host staging buffer [T][N] for coordinate transfers
@@ -817,6 +818,7 @@ int resident_prepare(sop_handle *h) {
   int occ = 0;
   CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->res_fn, pl.res_block, R.smem_bytes));
   if (occ < 1) return fail(SOP_E_CUDA, "resident kernel does not fit on an SM", h);
+  h->res_resident_ctas = occ * device_sm_count();          // CTAs of the first resident kernel the device holds at once
   if (pl.res2_ok) {
     h->res2_fn = res2_kernel(pl.comp, h->S.nat_eps != nullptr, pl.R2.P);
     CUDA_OK(cudaFuncSetAttribute(h->res2_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->R2.smem_bytes));
@@ -852,8 +854,8 @@ int resident_launch(sop_handle *h, int n, bool filter_last, bool filter_first) {
   // chained through `done` -- so every SM is busy until the last wave of slices.  A slice is what a separate launch of
   // slice_len steps would be (same prologue / epilogue, same bits); slice_len is a multiple of nb_interval.
   unsigned n_cta = (unsigned)(S.T * R.C);
-  if (R.C == 1 && !h->plan.res2_ok && !R.stream && S.T > device_sm_count() && !getenv("SOP_NO_SLICES")) {
-    const int sms = device_sm_count();
+  if (R.C == 1 && !h->plan.res2_ok && !R.stream && S.T > h->res_resident_ctas && !getenv("SOP_NO_SLICES")) {
+    const int sms = h->res_resident_ctas;                   // (CTA slots, not SMs, when several small CTAs share an SM)
     long long best_cost = 0; int best_len = 0;
     for (int len = 2 * nb; len < n; len += nb) {
       const long long slices = (n + len - 1) / len;
