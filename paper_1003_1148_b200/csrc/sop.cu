@@ -747,6 +747,18 @@ int persistent_launch(sop_handle *h, int n, bool filter_last) {
 // The register budget follows the block size (one CTA per SM: 65536 / threads): the instantiations for blocks of <= 832 and
 // <= 576 threads get 72 and 112 registers instead of 64, which takes address rematerialisation out of the pair loops
 // (cfg 2, 544 threads: 4.19 -> 3.98 us per step; cfg 3, 832 threads: 5.39 -> 5.35).  Same arithmetic, same bits.
+// FAST instantiations (the run-time switches of the step loop folded, see k_resident): the lane counts and block sizes the
+// auto plan gives large systems
+template <int G>
+const void *resident_fast_fn(bool comp, int block) {
+  if (block <= 576) return comp ? (const void *)k_resident<G, true, false, 576, true> : (const void *)k_resident<G, false, false, 576, true>;
+  if (block <= 832) return comp ? (const void *)k_resident<G, true, false, 832, true> : (const void *)k_resident<G, false, false, 832, true>;
+  return nullptr;
+}
+const void *resident_fast_kernel(int lanes, bool comp, int block) {
+  return lanes == 2 ? resident_fast_fn<2>(comp, block) : lanes == 4 ? resident_fast_fn<4>(comp, block) : nullptr;
+}
+
 template <int G>
 const void *resident_fn(bool comp, int block) {
   if constexpr (G <= 4) {
@@ -812,6 +824,8 @@ int resident_prepare(sop_handle *h) {
     k_transpose_nat<<<(h->S.N + 255) / 256, 256, 0, h->stream>>>(h->S, R);
   }
   h->res_fn = R.stream ? resident_stream_kernel(pl.res_lanes, pl.comp) : resident_kernel(pl.res_lanes, pl.comp, pl.res_block);
+  if (!R.stream && R.C > 1 && !R.implicit_l1 && R.nat_smem && !h->S.nat_eps && !h->S.taus && R.skew_ns == 0 && !getenv("SOP_NO_FAST"))
+    if (const void *f = resident_fast_kernel(pl.res_lanes, pl.comp, pl.res_block)) h->res_fn = f;
   CUDA_OK(cudaFuncSetAttribute(h->res_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, R.smem_bytes));
   const int loc_smem = ((h->S.N + 31) / 32) * 8 + R.chunk * 4;
   CUDA_OK(cudaFuncSetAttribute((const void *)k_localise, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(loc_smem, 1024)));

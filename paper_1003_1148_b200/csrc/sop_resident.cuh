@@ -268,7 +268,11 @@ __device__ __forceinline__ int lower_bound_dev(const int *__restrict__ a, int n,
 // update can be done in place --, and the lists live in global memory (L2-resident): rows are read coalesced, the partner
 // gathers stay in shared memory.
 // ------------------------------------------------------------------------------------------------
-template <int G, bool COMP, bool STREAM = false, int MAXT = 1024>
+// FAST: the switches the step loop would otherwise test at run time, every step, are constants of the common case -- several
+// chunks, explicit L1, natives in shared memory, one native eps, Philox noise, no skew hook (the host picks the instantiation):
+// shorter straight-line code per step, which a kernel whose every step walks through once-only code pays for in instruction
+// fetch.
+template <int G, bool COMP, bool STREAM = false, int MAXT = 1024, bool FAST = false>
 __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cur, unsigned long long step0, int n_steps,
                                                       int nb_interval, int filter_flags, uint32_t stamp0) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -324,7 +328,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
   const bool filter_last = filter_flags & 1, filter_first = filter_flags & 2;
   const int t = tc / R.C, c = tc - t * R.C;
   const int b0 = c * R.chunk, b1 = min(S.N, b0 + R.chunk), n_own = b1 - b0;
-  const bool multi = R.C > 1;
+  const bool multi = FAST || R.C > 1;
   const int n_halo = multi ? R.n_halo[tc] : 0;
   const int *__restrict__ hgid = R.halo_gid + (size_t)tc * R.halo_cap;
   const int HW = (n_halo + 31) >> 5;
@@ -374,7 +378,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
     plcnt_s[i] = R.implicit_l1 ? (unsigned short)0 : (unsigned short)S.pl_cnt[inst0 + b0 + i];
     const uint32_t tag = __float_as_uint(v.w);
     if (G > 1 && !(tag & TAG_FIXED)) {
-      const float3 gn = S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step0);
+      const float3 gn = !FAST && S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step0);
       sg[i] = make_float4(gn.x, gn.y, gn.z, 0.f);
     }
   }
@@ -456,7 +460,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
   // a3: Alg. 3 on the own rows, candidates and coordinates from shared memory
   auto filter_rows = [&](const float4 *P) {
     const uint32_t lt = (1u << wlane) - 1u;
-    if (R.implicit_l1 && n_own * 4 <= bd) {
+    if (!FAST && R.implicit_l1 && n_own * 4 <= bd) {
       // static all-pairs L1, few rows (cfg 0): one warp per row scans every j, ballot + prefix-popcount compaction
       for (int il = warp; il < n_own; il += nwarps) {
         const int gi = b0 + il;
@@ -473,7 +477,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
         if (n > cap_nb) { flag |= FLAG_NB_OVERFLOW; n = cap_nb; }
         if (wlane == 0) { cnt_s[il] = (unsigned short)n; for (int k4 = n; k4 & 3; ++k4) row[k4] = DUMMY; }
       }
-    } else if (R.implicit_l1) {
+    } else if (!FAST && R.implicit_l1) {
       // static all-pairs L1 (one chunk = the whole trajectory): L2 row of i = every j != i within R_nb that is not
       // bonded / native.  Candidates come from a cell grid over the chunk built here in shared memory (a1 in small:
       // bounding box -> count -> scan -> fill -> per-cell sort, so that the row order does not depend on atomics).
@@ -708,7 +712,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
   // ---- the steps
   ForceK K;
   K.k_fene = S.k_fene; K.inv_R0sq = S.inv_R0sq; K.eps12 = 12.0f * S.eps_native; K.c_rep_f = S.c_rep_f;
-  const float *nat_eps = S.nat_eps;
+  const float *nat_eps = FAST ? nullptr : S.nat_eps;
   int until_filter = nb_interval - (int)(step0 % (unsigned long long)nb_interval);
   bool have_full = true;                     // the whole halo of the current layer is already in shared memory (prologue)
   for (int k = 0; k < n_steps; ++k) {
@@ -797,7 +801,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
             }
           }
         }
-        else if (!nat_eps && R.nat_T) {
+        else if (!FAST && !nat_eps && R.nat_T) {
           // one-chunk trajectories with one lane per bead (cfg 1): the transposed table is read coalesced from L2, eight
           // independent entry loads in flight instead of one L2 round trip per native contact (same order of summation;
           // an entry past the end is the dummy slot with r0^2 = 0: its term is exactly zero)
@@ -818,7 +822,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
           }
         }
         else if (nat_eps) natives(std::true_type{}, std::false_type{});
-        else if (R.nat_smem) natives(std::false_type{}, std::true_type{});
+        else if (FAST || R.nat_smem) natives(std::false_type{}, std::true_type{});
         else natives(std::false_type{}, std::false_type{});
         // a6: non-native repulsion   V = eps_r (sigma/r)^6; four slots per 8-byte word (rows are padded to a multiple
         // of four with the dummy slot): one index load, four gathers in flight
@@ -855,7 +859,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
     const bool filt_due = until_filter == 1 && (k + 1 < n_steps || filter_last);   // the new layer is one every chunk filters on
     if (filt_due) fpar ^= 1u;
     uint4 *const xpub = filt_due ? (fpar ? xf1 : xf0) : xn;
-    if (R.skew_ns && tc == R.skew_chunk && step % (unsigned long long)R.skew_period == 0) __nanosleep((unsigned)R.skew_ns);
+    if (!FAST && R.skew_ns && tc == R.skew_chunk && step % (unsigned long long)R.skew_period == 0) __nanosleep((unsigned)R.skew_ns);
     for (int i = tid; i < n_own; i += bd) {
       const float4 ri = pc[i];
       const uint32_t tag = stag[i];
@@ -866,7 +870,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
         external_force_at(S, b0 + i, ri, tag, ext, fx, fy, fz, flag);
         float3 gn;
         if (G > 1) { const float4 g4 = gc[i]; gn = make_float3(g4.x, g4.y, g4.z); }
-        else gn = S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step);   // thread per bead already
+        else gn = !FAST && S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step);   // thread per bead already
         out = langevin_apply<COMP>(S, ri, gn, fx, fy, fz, COMP ? scarry + i : nullptr, flag, amp_tr);
       }
       pn[i] = out;
@@ -876,7 +880,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
       for (int i = bd - 1 - tid; i < n_own; i += bd) {
         const uint32_t tag = stag[i];
         if (!(tag & TAG_FIXED)) {
-          const float3 gn = S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step + 1);
+          const float3 gn = !FAST && S.taus ? gaussian3_taus(S.taus + inst0 + b0 + i) : gaussian3(S, tag & TAG_ID_MASK, traj, step + 1);
           gnx[i] = make_float4(gn.x, gn.y, gn.z, 0.f);
         }
       }

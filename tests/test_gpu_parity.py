@@ -343,6 +343,29 @@ def test_many_trajectories_sliced_launch_is_bit_identical(R_pl):
     assert np.abs(xa - o.get_coords()).max() <= 3e-3           # (230 steps: DESIGN.md section 8, "beyond 100 steps")
 
 
+def test_mode3_fast_instantiation_is_bit_identical():
+    """Several chunks, explicit L1, natives in shared memory, Philox, one native eps: the host picks the instantiation of the
+    resident kernel in which those run-time switches are compile-time constants (less once-per-step code).  Same arithmetic in
+    the same order: bit-identical to the general instantiation (SOP_NO_FAST), on a chunked small system with 2 and 4 lanes
+    (pulled + indented, compensated or not) and on the full 30,000-bead shell."""
+    def run(w, n, **var):
+        s = sop().from_workload(w, mode=3, **var); s.run(n)
+        out = (s.get_coords(), s.get_lists(2)[0], s.get_lists(2)[1], s.get_energies())
+        s.close()
+        return out
+    cases = [(gen.two_chains(150, 3, R_pl=20.0), 230, dict(chunk_beads=100, lanes_per_bead=4)),
+             (gen.two_chains(150, 3, R_pl=20.0), 230, dict(chunk_beads=150, lanes_per_bead=2, compensated=1)),
+             (gen.make_config(3), 200, {})]
+    for w, n, var in cases:
+        a = run(w, n, **var)
+        os.environ["SOP_NO_FAST"] = "1"
+        try:
+            b = run(w, n, **var)
+        finally:
+            del os.environ["SOP_NO_FAST"]
+        assert all(np.array_equal(x, y) for x, y in zip(a, b)), var
+
+
 def test_full_config1_batch_finite_pair_list():
     w = gen.config1(R_pl=20.0)
     T = 16
