@@ -747,16 +747,25 @@ int persistent_launch(sop_handle *h, int n, bool filter_last) {
 // The register budget follows the block size (one CTA per SM: 65536 / threads): the instantiations for blocks of <= 832 and
 // <= 576 threads get 72 and 112 registers instead of 64, which takes address rematerialisation out of the pair loops
 // (cfg 2, 544 threads: 4.19 -> 3.98 us per step; cfg 3, 832 threads: 5.39 -> 5.35).  Same arithmetic, same bits.
-// FAST instantiations (the run-time switches of the step loop folded, see k_resident): the lane counts and block sizes the
-// auto plan gives large systems
+// SPEC instantiations (the run-time switches of the step loop folded, see k_resident): 1 = several chunks, with the lane
+// counts and block sizes the auto plan gives large systems; 2 = one chunk per trajectory with the static all-pairs L1
 template <int G>
 const void *resident_fast_fn(bool comp, int block) {
-  if (block <= 576) return comp ? (const void *)k_resident<G, true, false, 576, true> : (const void *)k_resident<G, false, false, 576, true>;
-  if (block <= 832) return comp ? (const void *)k_resident<G, true, false, 832, true> : (const void *)k_resident<G, false, false, 832, true>;
+  if (block <= 576) return comp ? (const void *)k_resident<G, true, false, 576, 1> : (const void *)k_resident<G, false, false, 576, 1>;
+  if (block <= 832) return comp ? (const void *)k_resident<G, true, false, 832, 1> : (const void *)k_resident<G, false, false, 832, 1>;
   return nullptr;
 }
 const void *resident_fast_kernel(int lanes, bool comp, int block) {
   return lanes == 2 ? resident_fast_fn<2>(comp, block) : lanes == 4 ? resident_fast_fn<4>(comp, block) : nullptr;
+}
+const void *resident_fast1_kernel(int lanes, bool comp) {
+#ifdef SOP_DEV_MIN
+  if (lanes == 8) return nullptr;
+#else
+  if (lanes == 8) return comp ? (const void *)k_resident<8, true, false, 1024, 2> : (const void *)k_resident<8, false, false, 1024, 2>;
+#endif
+  if (lanes == 1) return comp ? (const void *)k_resident<1, true, false, 1024, 2> : (const void *)k_resident<1, false, false, 1024, 2>;
+  return nullptr;
 }
 
 template <int G>
@@ -824,8 +833,12 @@ int resident_prepare(sop_handle *h) {
     k_transpose_nat<<<(h->S.N + 255) / 256, 256, 0, h->stream>>>(h->S, R);
   }
   h->res_fn = R.stream ? resident_stream_kernel(pl.res_lanes, pl.comp) : resident_kernel(pl.res_lanes, pl.comp, pl.res_block);
-  if (!R.stream && R.C > 1 && !R.implicit_l1 && R.nat_smem && !h->S.nat_eps && !h->S.taus && R.skew_ns == 0 && !getenv("SOP_NO_FAST"))
-    if (const void *f = resident_fast_kernel(pl.res_lanes, pl.comp, pl.res_block)) h->res_fn = f;
+  if (!R.stream && !h->S.nat_eps && !h->S.taus && R.skew_ns == 0 && !getenv("SOP_NO_FAST")) {
+    const void *f = nullptr;
+    if (R.C > 1 && !R.implicit_l1 && R.nat_smem) f = resident_fast_kernel(pl.res_lanes, pl.comp, pl.res_block);
+    if (R.C == 1 && R.implicit_l1 && (pl.res_lanes == 1 ? R.nat_tpad > 0 : R.nat_smem != 0)) f = resident_fast1_kernel(pl.res_lanes, pl.comp);
+    if (f) h->res_fn = f;
+  }
   CUDA_OK(cudaFuncSetAttribute(h->res_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, R.smem_bytes));
   const int loc_smem = ((h->S.N + 31) / 32) * 8 + R.chunk * 4;
   CUDA_OK(cudaFuncSetAttribute((const void *)k_localise, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(loc_smem, 1024)));

@@ -268,11 +268,12 @@ __device__ __forceinline__ int lower_bound_dev(const int *__restrict__ a, int n,
 // update can be done in place --, and the lists live in global memory (L2-resident): rows are read coalesced, the partner
 // gathers stay in shared memory.
 // ------------------------------------------------------------------------------------------------
-// FAST: the switches the step loop would otherwise test at run time, every step, are constants of the common case -- several
-// chunks, explicit L1, natives in shared memory, one native eps, Philox noise, no skew hook (the host picks the instantiation):
-// shorter straight-line code per step, which a kernel whose every step walks through once-only code pays for in instruction
-// fetch.
-template <int G, bool COMP, bool STREAM = false, int MAXT = 1024, bool FAST = false>
+// SPEC: the switches the step loop would otherwise test at run time, every step, are constants of the two common cases (the
+// host picks the instantiation; 0 = general).  1: several chunks, explicit L1, natives in shared memory.  2: one chunk per
+// trajectory with the static all-pairs L1, natives transposed in global memory (one lane per bead) or in shared memory
+// (several lanes).  Both: one native eps, Philox noise, no skew hook.  Less straight-line code per step, which a kernel whose
+// every step walks through once-only code pays for in instruction fetch.
+template <int G, bool COMP, bool STREAM = false, int MAXT = 1024, int SPEC = 0>
 __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cur, unsigned long long step0, int n_steps,
                                                       int nb_interval, int filter_flags, uint32_t stamp0) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -328,7 +329,8 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
   const bool filter_last = filter_flags & 1, filter_first = filter_flags & 2;
   const int t = tc / R.C, c = tc - t * R.C;
   const int b0 = c * R.chunk, b1 = min(S.N, b0 + R.chunk), n_own = b1 - b0;
-  const bool multi = FAST || R.C > 1;
+  constexpr bool FAST = SPEC != 0;
+  const bool multi = SPEC == 1 || (SPEC == 0 && R.C > 1);
   const int n_halo = multi ? R.n_halo[tc] : 0;
   const int *__restrict__ hgid = R.halo_gid + (size_t)tc * R.halo_cap;
   const int HW = (n_halo + 31) >> 5;
@@ -460,7 +462,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
   // a3: Alg. 3 on the own rows, candidates and coordinates from shared memory
   auto filter_rows = [&](const float4 *P) {
     const uint32_t lt = (1u << wlane) - 1u;
-    if (!FAST && R.implicit_l1 && n_own * 4 <= bd) {
+    if ((SPEC == 2 || (SPEC == 0 && R.implicit_l1)) && n_own * 4 <= bd) {
       // static all-pairs L1, few rows (cfg 0): one warp per row scans every j, ballot + prefix-popcount compaction
       for (int il = warp; il < n_own; il += nwarps) {
         const int gi = b0 + il;
@@ -477,7 +479,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
         if (n > cap_nb) { flag |= FLAG_NB_OVERFLOW; n = cap_nb; }
         if (wlane == 0) { cnt_s[il] = (unsigned short)n; for (int k4 = n; k4 & 3; ++k4) row[k4] = DUMMY; }
       }
-    } else if (!FAST && R.implicit_l1) {
+    } else if (SPEC == 2 || (SPEC == 0 && R.implicit_l1)) {
       // static all-pairs L1 (one chunk = the whole trajectory): L2 row of i = every j != i within R_nb that is not
       // bonded / native.  Candidates come from a cell grid over the chunk built here in shared memory (a1 in small:
       // bounding box -> count -> scan -> fill -> per-cell sort, so that the row order does not depend on atomics).
@@ -801,7 +803,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
             }
           }
         }
-        else if (!FAST && !nat_eps && R.nat_T) {
+        else if (SPEC == 2 ? G == 1 : SPEC == 0 && !nat_eps && R.nat_T) {
           // one-chunk trajectories with one lane per bead (cfg 1): the transposed table is read coalesced from L2, eight
           // independent entry loads in flight instead of one L2 round trip per native contact (same order of summation;
           // an entry past the end is the dummy slot with r0^2 = 0: its term is exactly zero)
@@ -822,7 +824,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
           }
         }
         else if (nat_eps) natives(std::true_type{}, std::false_type{});
-        else if (FAST || R.nat_smem) natives(std::false_type{}, std::true_type{});
+        else if (SPEC == 1 || (SPEC == 2 && G > 1) || (SPEC == 0 && R.nat_smem)) natives(std::false_type{}, std::true_type{});
         else natives(std::false_type{}, std::false_type{});
         // a6: non-native repulsion   V = eps_r (sigma/r)^6; four slots per 8-byte word (rows are padded to a multiple
         // of four with the dummy slot): one index load, four gathers in flight

@@ -344,18 +344,21 @@ def test_many_trajectories_sliced_launch_is_bit_identical(R_pl):
 
 
 def test_mode3_fast_instantiation_is_bit_identical():
-    """Several chunks, explicit L1, natives in shared memory, Philox, one native eps: the host picks the instantiation of the
-    resident kernel in which those run-time switches are compile-time constants (less once-per-step code).  Same arithmetic in
-    the same order: bit-identical to the general instantiation (SOP_NO_FAST), on a chunked small system with 2 and 4 lanes
-    (pulled + indented, compensated or not) and on the full 30,000-bead shell."""
-    def run(w, n, **var):
-        s = sop().from_workload(w, mode=3, **var); s.run(n)
+    """Philox, one native eps and either (1) several chunks, explicit L1, natives in shared memory or (2) one chunk per
+    trajectory with the static all-pairs L1: the host picks an instantiation of the resident kernel in which those run-time
+    switches are compile-time constants (less once-per-step code).  Same arithmetic in the same order: bit-identical to the
+    general instantiation (SOP_NO_FAST), on chunked small systems with 2 and 4 lanes, the full 30,000-bead shell, config 0
+    (8 lanes, one chunk) and a one-lane batch with the transposed native table."""
+    def run(w, n, n_traj=None, **var):
+        s = sop().from_workload(w, n_traj=n_traj, mode=3, **var); s.run(n)
         out = (s.get_coords(), s.get_lists(2)[0], s.get_lists(2)[1], s.get_energies())
         s.close()
         return out
     cases = [(gen.two_chains(150, 3, R_pl=20.0), 230, dict(chunk_beads=100, lanes_per_bead=4)),
              (gen.two_chains(150, 3, R_pl=20.0), 230, dict(chunk_beads=150, lanes_per_bead=2, compensated=1)),
-             (gen.make_config(3), 200, {})]
+             (gen.make_config(3), 200, {}),
+             (gen.make_config(0), 230, {}),                                      # one chunk, static L1, 8 lanes
+             (gen.globule(700, 5), 130, dict(lanes_per_bead=1, n_traj=3))]      # one chunk, static L1, one lane, transposed natives
     for w, n, var in cases:
         a = run(w, n, **var)
         os.environ["SOP_NO_FAST"] = "1"
