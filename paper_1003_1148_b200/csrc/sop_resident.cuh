@@ -643,27 +643,30 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
           // the (up to 32 LPR) words of this round are split evenly: at most 32 words = 64 candidates per lane
           const int rw0 = r * 32 * LPR, rwn = min(32 * LPR, nw - rw0), per = (max(rwn, 0) + LPR - 1) / LPR;
           const int w0 = rw0 + flane * per;
-          unsigned long long mask = 0ull;
+          // survivors as two 32-bit masks (low / high slot of word k2 at bit k2): one predicated OR per candidate
+          uint32_t ma = 0u, mb = 0u, bit = 1u;
           const int wend = min(per, rwn - flane * per);
 #pragma unroll 4
           for (int k2 = 0; k2 < wend; ++k2) {
             const uint32_t u = word(w0 + k2);
             const bool pa = pred32(ri, P[u & 0xFFFFu], S.R_nb2);
             const bool pb = 2 * (w0 + k2) + 1 < cnt1 && pred32(ri, P[u >> 16], S.R_nb2);
-            mask |= (unsigned long long)(pa ? 1u : 0u) << (2 * k2);
-            mask |= (unsigned long long)(pb ? 1u : 0u) << (2 * k2 + 1);
+            if (pa) ma |= bit;
+            if (pb) mb |= bit;
+            bit <<= 1;
           }
-          const int mine = __popcll(mask);
+          const int mine = __popc(ma) + __popc(mb);
           int incl = mine;
           for (int o = 1; o < LPR; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o, LPR); if (flane >= o) incl += v; }
           const int total = __shfl_sync(0xffffffffu, incl, LPR - 1, LPR);
           int at = n + incl - mine;
-          while (mask) {
-            const int bit = __ffsll((long long)mask) - 1;
-            mask &= mask - 1;
-            const uint32_t u = word(w0 + (bit >> 1));
-            if (at < cap_nb) row[at] = (unsigned short)((bit & 1) ? (u >> 16) : (u & 0xFFFFu));
-            ++at;
+          uint32_t many = ma | mb;
+          while (many) {                               // words with a survivor, in row order: low slot before high slot
+            const int k2 = __ffs((int)many) - 1;
+            many &= many - 1;
+            const uint32_t u = word(w0 + k2);
+            if ((ma >> k2) & 1u) { if (at < cap_nb) row[at] = (unsigned short)(u & 0xFFFFu); ++at; }
+            if ((mb >> k2) & 1u) { if (at < cap_nb) row[at] = (unsigned short)(u >> 16); ++at; }
           }
           n += total;
         }
