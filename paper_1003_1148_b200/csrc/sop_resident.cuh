@@ -309,20 +309,33 @@ __global__ void __launch_bounds__(MAXT, 1) k_resident(SysDev S, ResDev R, int cu
     __syncthreads();
     const int n_tc = S.T * R.C, n_total = n_steps;
     slice = s_ticket / n_tc; tc = s_ticket - slice * n_tc;
+    if (s_ticket < 0 || (long long)slice * R.slice_len >= n_total) return;      // (a ticket outside the grid's range: nothing to do)
     step0 += (unsigned long long)slice * (unsigned long long)R.slice_len;
     n_steps = min(R.slice_len, n_total - slice * R.slice_len);
     const bool last = (slice + 1) * R.slice_len >= n_total;
     // (slice_len is a multiple of nb_interval: the filter due at the end of an inner slice runs inside it)
     filter_flags = (last ? (filter_flags & 1) : 1) | (slice == 0 ? (filter_flags & 2) : 0);
     if (slice > 0) {
+      // bounded like every other wait of this kernel (seconds: a lost ticket order would be a protocol fault): the flag is
+      // raised, this slice and -- through the abort word -- every later one is skipped, the launch ends with SOP_E_CUDA
+      __shared__ int s_ok;
       if (threadIdx.x == 0) {
-        int seen;
-        do {
+        volatile int *abort_word = S.flags + 1;
+        int seen, ok = 1;
+        for (unsigned spins = 0;; ++spins) {
           asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(R.done + tc) : "memory");
-          if (seen < slice) __nanosleep(200);
-        } while (seen < slice);
+          if (seen >= slice) break;
+          if (*abort_word) { ok = 0; break; }
+          if (spins >= XCH_SPIN_LIMIT) { atomicOr(S.flags, FLAG_EXCHANGE_TIMEOUT); *abort_word = 1; __threadfence(); ok = 0; break; }
+          __nanosleep(200);
+        }
+        s_ok = ok;
       }
       __syncthreads();
+      if (!s_ok) {
+        if (threadIdx.x == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(R.done + tc), "r"(slice + 1) : "memory");
+        return;
+      }
       __threadfence();                         // every thread reads what the previous slice wrote (no stale L1 lines)
     }
   }
