@@ -181,6 +181,13 @@ int sop_device_coords(sop_handle *, void **d_float4_out, int32_t *perm_out);
  * steps per time slice of the most recent SLICED mode-3 launch (0: none so far; many one-chunk trajectories,
  * PAPER.md:292), reserved. */
 int sop_get_config(sop_handle *, int32_t out[12]);
+/* Launch planning of the many-runs batch (many independent trajectories of a small system in one launch), host
+ * arithmetic only, no device call: the number of Langevin steps per TIME SLICE a mode-3 launch of n_steps steps over n_traj
+ * one-chunk trajectories is cut into when the device holds cta_slots resident CTAs at once (one CTA per slice and trajectory,
+ * handed out slice-major by a ticket, so that no SM idles through a partly empty last wave); 0 = not sliced (n_traj <=
+ * cta_slots, a short launch, or less than 3 % to gain).  A positive result is a multiple of nb_interval, at least
+ * 2 * nb_interval and less than n_steps.  Bad arguments (anything < 1) return 0. */
+int32_t sop_plan_slices(int32_t n_steps, int32_t nb_interval, int32_t n_traj, int32_t cta_slots);
 /* Kernel timing for the bench (CUDA events on the handle's stream around groups of launches of one kind).
  * sop_get_profile synchronises, fills out[0..2] = ms spent in {step kernels, L2 filter kernels, L1 build kernels},
  * out[3..5] = number of timed spans of each kind, out[6] = Langevin steps covered by the step spans, and resets. */

@@ -882,16 +882,8 @@ int resident_launch(sop_handle *h, int n, bool filter_last, bool filter_first) {
   // slice_len steps would be (same prologue / epilogue, same bits); slice_len is a multiple of nb_interval.
   unsigned n_cta = (unsigned)(S.T * R.C);
   if (R.C == 1 && !h->plan.res2_ok && !R.stream && S.T > h->res_resident_ctas && !getenv("SOP_NO_SLICES")) {
-    const int sms = h->res_resident_ctas;                   // (CTA slots, not SMs, when several small CTAs share an SM)
-    long long best_cost = 0; int best_len = 0;
-    for (int len = 2 * nb; len < n; len += nb) {
-      const long long slices = (n + len - 1) / len;
-      const long long waves = (slices * S.T + sms - 1) / sms;
-      const long long cost = waves * (2 * len + 7);           // (a slice costs about 3.5 steps of prologue + epilogue: measured)
-      if (!best_len || cost < best_cost) { best_cost = cost; best_len = len; }
-    }
-    const long long plain = (long long)((S.T + sms - 1) / sms) * (2 * n + 7);
-    if (best_len && best_cost * 100 < plain * 97) {
+    const int best_len = sop_plan_slices(n, nb, S.T, h->res_resident_ctas);   // (CTA slots, not SMs, when small CTAs share an SM)
+    if (best_len > 0) {
       R.slice_len = best_len;
       h->last_slice_len = best_len;
       n_cta = (unsigned)(((n + best_len - 1) / best_len) * S.T);
@@ -994,6 +986,24 @@ int noalloc_scratch(sop_handle *h, double **out) {
 
 // =====================================================================================================
 extern "C" {
+
+// Steps per time slice of a launch of n_steps Langevin steps over n_traj one-chunk trajectories when the device holds
+// cta_slots CTAs of the resident kernel at once; 0 = one CTA per trajectory for the whole launch.  Host arithmetic only.
+// Cost model: waves of CTAs x (slice length + 3.5 steps of measured prologue / epilogue cost per slice); slices are multiples
+// of nb_interval and at least two filter intervals long; slicing must save 3 % to be chosen.
+int32_t sop_plan_slices(int32_t n_steps, int32_t nb_interval, int32_t n_traj, int32_t cta_slots) {
+  if (n_steps < 1 || nb_interval < 1 || n_traj < 1 || cta_slots < 1 || n_traj <= cta_slots) return 0;
+  long long best_cost = 0; int best_len = 0;
+  for (int len = 2 * nb_interval; len < n_steps; len += nb_interval) {
+    const long long slices = (n_steps + len - 1) / len;
+    const long long waves = (slices * n_traj + cta_slots - 1) / cta_slots;
+    const long long cost = waves * (2LL * len + 7);
+    if (!best_len || cost < best_cost) { best_cost = cost; best_len = len; }
+  }
+  const long long plain = (long long)((n_traj + cta_slots - 1) / cta_slots) * (2LL * n_steps + 7);
+  return best_len && best_cost * 100 < plain * 97 ? best_len : 0;
+}
+
 
 const char *sop_last_error(sop_handle *h) { return h ? h->last_error.c_str() : g_last_error.c_str(); }
 

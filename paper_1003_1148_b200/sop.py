@@ -20,7 +20,7 @@ SYMBOLS = ["sop_query_workspace", "sop_create", "sop_destroy", "sop_run", "sop_s
            "sop_set_coords", "sop_get_energies", "sop_get_observables", "sop_get_forces", "sop_get_lists", "sop_get_step", "sop_set_step",
            "sop_device_coords", "sop_get_config", "sop_set_profiling", "sop_get_profile", "sop_last_error",
            "sop_set_observable_stride", "sop_get_observable_series", "sop_replica_exchange", "sop_get_temperatures",
-           "sop_energies_noalloc"]
+           "sop_energies_noalloc", "sop_plan_slices"]
 
 
 class _Topology(C.Structure):
@@ -86,6 +86,7 @@ def lib():
         L.sop_set_step.argtypes = [vp, i64]
         L.sop_device_coords.argtypes = [vp, C.POINTER(vp), vp]
         L.sop_get_config.argtypes = [vp, vp]
+        L.sop_plan_slices.argtypes = [i32, i32, i32, i32]; L.sop_plan_slices.restype = i32
         L.sop_set_profiling.argtypes = [vp, i32]
         L.sop_get_profile.argtypes = [vp, vp]
         L.sop_last_error.argtypes = [vp]; L.sop_last_error.restype = C.c_char_p

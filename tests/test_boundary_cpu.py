@@ -50,6 +50,32 @@ def test_query_workspace_is_host_only_and_validates():
     assert rc_s == 0 and rc_f == 0 and n_f < n_s
 
 
+def test_slice_planner_host_logic():
+    """sop_plan_slices (host arithmetic behind the sliced launches of the many-runs batch): no slicing when every trajectory
+    has a CTA slot or the launch is short; otherwise a multiple of nb_interval, at least two filter intervals, shorter than the
+    launch, and with fewer waves x (slice + overhead) than the plain launch; config 1's case (256 trajectories, 148 slots,
+    1000 steps) is sliced."""
+    from paper_1003_1148_b200 import sop
+    plan = sop.lib().sop_plan_slices
+    assert plan(1000, 10, 148, 148) == 0 and plan(1000, 10, 1, 148) == 0          # a slot for everyone
+    assert plan(25, 10, 256, 148) == 0                                              # too short to cut
+    for bad in ((0, 10, 256, 148), (1000, 0, 256, 148), (1000, 10, 0, 148), (1000, 10, 256, 0)):
+        assert plan(*bad) == 0
+    L = plan(1000, 10, 256, 148)
+    assert L > 0
+    for n, nb, T, slots in ((1000, 10, 256, 148), (200, 10, 256, 148), (100, 10, 160, 148), (230, 10, 160, 148),
+                            (5000, 25, 1000, 296), (100000, 10, 300, 148)):
+        L = plan(n, nb, T, slots)
+        if L == 0:
+            continue
+        assert L % nb == 0 and 2 * nb <= L < n
+        slices = -(-n // L)
+        waves, plain_waves = -(-slices * T // slots), -(-T // slots)
+        assert waves * (2 * L + 7) * 100 < plain_waves * (2 * n + 7) * 97
+    # more slots than a one-CTA-per-SM kernel has: several small CTAs per SM are counted as slots
+    assert plan(1000, 10, 256, 296) == 0
+
+
 def test_struct_layout_matches_header():
     """Field order of the ctypes mirror follows the declaration order of sop_params in include/sop.h."""
     from paper_1003_1148_b200 import sop
